@@ -1,0 +1,132 @@
+"""CPU oracle of the CBM-MUCH first-level J/psi selection -- TEST INFRASTRUCTURE.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference leg
+may import this package.  It is independent of the CUDA path (no shared code, headers,
+helpers or tables); the product never routes through it.
+
+    run(...)            -> oracle/cbm_oracle.c   (the definition as nested loops, int64)
+    run_slope_sorted()  -> oracle/slope_sorted.c (independent sorted/multiplicity route; a pin)
+    brute_force         -> oracle/brute_force.py (no short-circuit, explicit S-tuples; a pin)
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB = os.path.join(_HERE, "liboracle.so")
+_SRCS = [os.path.join(_HERE, "cbm_oracle.c"), os.path.join(_HERE, "slope_sorted.c")]
+MAX_LAYERS = 24
+
+
+class Geometry(ctypes.Structure):
+    _fields_ = [
+        ("n_stations", ctypes.c_uint32),
+        ("layer_z", ctypes.c_int32 * MAX_LAYERS),
+        ("win_in_num", ctypes.c_uint32), ("win_in_den", ctypes.c_uint32),
+        ("win_link_num", ctypes.c_uint32), ("win_link_den", ctypes.c_uint32),
+        ("min_candidates", ctypes.c_uint32),
+    ]
+
+
+def geometry(layer_z, win_in=(1, 100), win_link=(2, 100), min_candidates=2) -> Geometry:
+    g = Geometry()
+    assert len(layer_z) % 3 == 0 and 3 <= len(layer_z) <= MAX_LAYERS
+    g.n_stations = len(layer_z) // 3
+    for i, z in enumerate(layer_z):
+        g.layer_z[i] = int(z)
+    g.win_in_num, g.win_in_den = win_in
+    g.win_link_num, g.win_link_den = win_link
+    g.min_candidates = min_candidates
+    return g
+
+
+def build(force: bool = False) -> str:
+    """gcc -O2 (the paper's CPU flags, minus -march=native so the .so is portable)."""
+    newest = max(os.path.getmtime(s) for s in _SRCS)
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < newest:
+        subprocess.run(["gcc", "-O2", "-fPIC", "-shared", "-std=c11", "-o", _LIB] + _SRCS, check=True)
+    return _LIB
+
+
+_lib = None
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        build()
+        lib = ctypes.CDLL(_LIB)
+        vp, u64 = ctypes.c_void_p, ctypes.c_uint64
+        lib.cbm_oracle_run.restype = ctypes.c_int
+        lib.cbm_oracle_run.argtypes = [ctypes.POINTER(Geometry), vp, vp, vp, u64, u64, u64, vp, vp, vp]
+        lib.cbm_oracle_run_list.restype = ctypes.c_int
+        lib.cbm_oracle_run_list.argtypes = [ctypes.POINTER(Geometry), vp, vp, vp, vp, u64, u64, vp, vp, vp]
+        lib.cbm_slope_sorted_run.restype = ctypes.c_int
+        lib.cbm_slope_sorted_run.argtypes = [ctypes.POINTER(Geometry), vp, vp, vp, u64, u64, vp, vp, vp, vp]
+        _lib = lib
+    return _lib
+
+
+def _check_inputs(x, y, off):
+    x = np.ascontiguousarray(x, dtype=np.int32)
+    y = np.ascontiguousarray(y, dtype=np.int32)
+    off = np.ascontiguousarray(off, dtype=np.uint32)
+    return x, y, off
+
+
+def run(geo: Geometry, x, y, off, e_begin=0, e_end=None, max_list_entries=0):
+    """Oracle over events [e_begin, e_end).  Returns (n_triplets[n,S], n_candidates[n], accept[n])."""
+    lib = _load()
+    x, y, off = _check_inputs(x, y, off)
+    S = geo.n_stations
+    n_events = (off.size - 1) // (3 * S)
+    e_end = n_events if e_end is None else e_end
+    n = e_end - e_begin
+    nt = np.zeros((max(n, 0), S), dtype=np.uint32)
+    nc = np.zeros(max(n, 0), dtype=np.uint32)
+    ac = np.zeros(max(n, 0), dtype=np.uint8)
+    rc = lib.cbm_oracle_run(ctypes.byref(geo), x.ctypes.data, y.ctypes.data, off.ctypes.data, e_begin, e_end,
+                            max_list_entries, nt.ctypes.data, nc.ctypes.data, ac.ctypes.data)
+    if rc != 0:
+        raise RuntimeError(f"cbm_oracle_run failed: {rc}")
+    return nt, nc, ac
+
+
+def run_list(geo: Geometry, x, y, off, event_ids, max_list_entries=0):
+    """Oracle over a list of event ids (sampled parity at full size)."""
+    lib = _load()
+    x, y, off = _check_inputs(x, y, off)
+    ids = np.ascontiguousarray(event_ids, dtype=np.uint64)
+    S = geo.n_stations
+    nt = np.zeros((ids.size, S), dtype=np.uint32)
+    nc = np.zeros(ids.size, dtype=np.uint32)
+    ac = np.zeros(ids.size, dtype=np.uint8)
+    rc = lib.cbm_oracle_run_list(ctypes.byref(geo), x.ctypes.data, y.ctypes.data, off.ctypes.data,
+                                 ids.ctypes.data, ids.size, max_list_entries,
+                                 nt.ctypes.data, nc.ctypes.data, ac.ctypes.data)
+    if rc != 0:
+        raise RuntimeError(f"cbm_oracle_run_list failed: {rc}")
+    return nt, nc, ac
+
+
+def run_slope_sorted(geo: Geometry, x, y, off, e_begin=0, e_end=None):
+    """Independent sorted/multiplicity implementation.  Returns (n_triplets, n_candidates, accept, n_eval)."""
+    lib = _load()
+    x, y, off = _check_inputs(x, y, off)
+    S = geo.n_stations
+    n_events = (off.size - 1) // (3 * S)
+    e_end = n_events if e_end is None else e_end
+    n = e_end - e_begin
+    nt = np.zeros((max(n, 0), S), dtype=np.uint32)
+    nc = np.zeros(max(n, 0), dtype=np.uint32)
+    ac = np.zeros(max(n, 0), dtype=np.uint8)
+    ne = ctypes.c_uint64(0)
+    rc = lib.cbm_slope_sorted_run(ctypes.byref(geo), x.ctypes.data, y.ctypes.data, off.ctypes.data, e_begin, e_end,
+                                  nt.ctypes.data, nc.ctypes.data, ac.ctypes.data, ctypes.byref(ne))
+    if rc != 0:
+        raise RuntimeError(f"cbm_slope_sorted_run failed: {rc}")
+    return nt, nc, ac, int(ne.value)
