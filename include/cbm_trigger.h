@@ -1,0 +1,160 @@
+/* cbm_trigger.h -- C ABI of libcbmtrigger.so
+ *
+ * B200-native (sm_100a) first-level J/psi -> mu+ mu- event selection for the CBM muon
+ * chambers (MUCH), after Singhal, Chattopadhyay, Friese, "Investigation of heterogeneous
+ * computing platforms for real-time data analysis in the CBM experiment" (arxiv 1810.11966;
+ * PAPER.md).  Plain C: plain pointers and sizes, no exceptions and no C++/torch types cross
+ * this boundary.  Every pointer argument says HOST or DEVICE.
+ *
+ * What is computed (section 3.2 steps 1-3, with the integer slope windows and
+ * the cross-station linking BASELINE.json's north_star fixes):
+ *
+ *   compat(h in layer A, g in layer B; a/b) :=  b*|x_h*z_B - x_g*z_A| <= a*z_A*z_B
+ *                                           and b*|y_h*z_B - y_g*z_A| <= a*z_A*z_B       (int64, exact)
+ *   T_s  := { (h0,h1,h2) in layer0 x layer1 x layer2 of station s : all three pairs compat under win_in }
+ *           -- PAPER.md:73 "Create all possible triplets of hits ..., with one hit from each layer";
+ *              the triplet and the event vertex (0,0) lie on a straight line in x-z and y-z
+ *   link(t in T_s, u in T_{s+1}) := compat(t.h1, u.h1; win_link)            (middle-layer hits)
+ *   candidates := number of tuples (t_0, ..., t_{S-1}), t_s in T_s, consecutive ones linked
+ *   n_triplets[e*S+s] = min(2^32-1, |T_s|);  n_candidates[e] = min(2^32-1, candidates)
+ *   accept[e] = n_candidates[e] >= min_candidates        -- PAPER.md:88 "Select the event if it contains at
+ *                                                            least two triplets ..." (generalised to candidates)
+ *
+ * Data layout ("separate data containers for each coordinate axis", one record per batch):
+ *   x[n_hits], y[n_hits]   int32, 10-um units; hits of event e, layer l (= 3*station + layer-in-station)
+ *                          are x[off[e*L+l] .. off[e*L+l+1]);  z is a per-layer constant (config)
+ *   off[n_events*L + 1]    uint32, off[0] = 0, non-decreasing, off[n_events*L] = n_hits, L = 3*n_stations
+ *
+ * Error behaviour: every call returns CBM_OK (0) or a negative code; on error nothing is enqueued and the
+ * handle stays usable.  cbm_trigger_last_error() returns a handle-owned message for the last failure.
+ * A handle is not thread-safe; different slots may be driven from one thread as a software pipeline.
+ *
+ * Arithmetic range: the device evaluates |x_h*z_B - x_g*z_A| <= floor(a*z_A*z_B/b) in int64, which is exact
+ * for any int32 x, y and 0 < z <= 2^23 (|D| < 2^56).  (The CPU oracle's b*|D| form needs |x|,|y| <= 2^23.)
+ */
+#ifndef CBM_TRIGGER_H
+#define CBM_TRIGGER_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define CBM_TRIGGER_MAX_STATIONS 8
+#define CBM_TRIGGER_MAX_LAYERS 24
+#define CBM_TRIGGER_MAX_HITS_PER_LAYER 4096
+#define CBM_TRIGGER_MAX_SLOTS 4
+#define CBM_TRIGGER_N_KERNELS 4 /* tile, team_M, team_H, team_G (see cbm_trigger_stats_t) */
+
+enum {
+  CBM_OK = 0,
+  CBM_ERR_INVALID_ARG = -1, /* null pointer, bad struct_size, S out of range, z not positive/increasing, den = 0 */
+  CBM_ERR_RANGE = -2,       /* offsets not monotone / beyond n_hits, a layer above max_hits_per_layer (found on
+                               the device during run, reported by fetch_results / device_status) */
+  CBM_ERR_CAPACITY = -3,    /* n_events / n_hits beyond the capacity given at create */
+  CBM_ERR_STATE = -4,       /* run before upload, fetch before run, slot out of range */
+  CBM_ERR_CUDA = -5         /* CUDA runtime failure (no device, out of memory, launch failure) */
+};
+
+typedef struct cbm_trigger cbm_trigger_t; /* opaque; owned by the caller via create/destroy */
+
+typedef struct {
+  uint32_t struct_size;  /* = sizeof(cbm_trigger_config_t) */
+  uint32_t n_stations;   /* S, 1..8; three layers per station */
+  int32_t  layer_z[CBM_TRIGGER_MAX_LAYERS]; /* z of layer 3*s+l, 10-um units, 0 < z <= 2^23, strictly increasing */
+  uint32_t win_in_num, win_in_den;     /* in-station slope window a/b (half-width, closed); 0 < den <= 4096, num <= den */
+  uint32_t win_link_num, win_link_den; /* cross-station window a/b, same limits */
+  uint32_t min_candidates;             /* accept iff n_candidates >= this (2) */
+  uint32_t max_events;                 /* capacity of one slot, in events */
+  uint64_t max_hits;                   /* capacity of one slot, in hits; < 2^32 */
+  uint32_t max_hits_per_layer;         /* 1..4096; an event with a fuller layer is rejected (CBM_ERR_RANGE) */
+  uint32_t n_slots;                    /* 0..4 slots of (pinned host + device) buffers; 2 = double buffering.
+                                          0: only cbm_trigger_run_device() is usable (caller owns all buffers) */
+  int32_t  device;                     /* CUDA ordinal */
+  uint32_t slope_range_milli;          /* tuning hint, never changes results: hits are binned over slopes
+                                          |x/z|,|y/z| <= this/1000 (outliers share the edge bins). 0 = 400 */
+  uint32_t tiny_max_layer_hits;        /* tuning: events whose fullest layer holds <= this many hits (and that fit
+                                          the tile) take the thread-per-station path. 0 = default (24); max 32 */
+  uint32_t flags;                      /* CBM_FLAG_* */
+} cbm_trigger_config_t;
+
+#define CBM_FLAG_PROFILE 1u      /* record CUDA events around every kernel (cbm_trigger_get_stats: kernel_ms) */
+#define CBM_FLAG_NO_TINY_PATH 2u /* tuning/testing: route every event through the team kernels */
+
+typedef struct {
+  uint32_t struct_size;
+  uint32_t n_events;
+  uint64_t n_hits;
+  uint32_t n_class[4];     /* events handled by: [0] tile kernel (tiny), [1] team_M, [2] team_H, [3] team_G */
+  uint32_t n_invalid;      /* events rejected on the device (bad offsets / layer too full); their outputs are 0 */
+  uint32_t first_invalid;  /* smallest such event index, 0xFFFFFFFF if none */
+  uint32_t n_launches;     /* kernels launched by the last run of this slot */
+  float    kernel_ms[CBM_TRIGGER_N_KERNELS]; /* CBM_FLAG_PROFILE only: device time of each kernel, else 0 */
+  float    h2d_ms, d2h_ms; /* CBM_FLAG_PROFILE only */
+} cbm_trigger_stats_t;
+
+/* Creates a handle: validates cfg (CBM_ERR_INVALID_ARG before any CUDA call), selects cfg->device, allocates
+ * n_slots x (pinned HOST staging + DEVICE arrays + result buffers) and the scheduler's device scratch, creates
+ * the H2D / compute / D2H streams.  *out is written only on success.  cfg: HOST. */
+int cbm_trigger_create(const cbm_trigger_config_t* cfg, cbm_trigger_t** out);
+
+/* Frees everything the handle owns (waits for its streams first).  NULL is allowed. */
+void cbm_trigger_destroy(cbm_trigger_t* h);
+
+/* Zero-copy staging: HOST pointers into the slot's pinned buffers (owned by the handle; capacity max_hits int32
+ * for x and y, max_events*L+1 uint32 for off).  A producer (DAQ / generator) writes a batch there and then calls
+ * upload_events with these same pointers, which skips the staging memcpy.  (data are delivered
+ * into host memory, then transferred.) */
+int cbm_trigger_host_buffers(cbm_trigger_t* h, uint32_t slot, int32_t** x, int32_t** y, uint32_t** off);
+
+/* a1+a2: enqueue the H2D copy of one batch into `slot` on the slot's copy stream.
+ * x, y: HOST, n_hits int32 each.  off: HOST, n_events*L+1 uint32 (layout above).  If the pointers are not the
+ * slot's own pinned buffers, the data are first memcpy'd into them, so caller memory may be reused on return.
+ * Checks on the host, O(1): capacity, off[0] == 0, off[n_events*L] == n_hits.  The O(E*L) structural checks
+ * (monotone offsets, per-layer cap) run on the device inside `run`.  Waits for the slot's previous use.
+ * PAPER.md:160-161 "allocate memory on the device ... transfer the data from host to device". */
+int cbm_trigger_upload_events(cbm_trigger_t* h, uint32_t slot, uint32_t n_events, uint64_t n_hits,
+                              const int32_t* x, const int32_t* y, const uint32_t* off);
+
+/* a3-a8: enqueue the selection kernels for the batch in `slot` after its H2D, and the D2H of the results after
+ * the kernels (separate streams, event-ordered).  Returns immediately.
+ * PAPER.md:162-163 "launch the kernel ... events are processed in parallel". */
+int cbm_trigger_run(cbm_trigger_t* h, uint32_t slot);
+
+/* a9: blocks until the slot's results are in pinned host memory, then copies them to the caller's HOST arrays:
+ * n_triplets[n_events*S] (may be NULL), n_candidates[n_events], accept[n_events] (may be NULL).
+ * Returns CBM_ERR_RANGE if the device rejected any event (outputs of those events are 0, all others are valid;
+ * last_error names the first one).  PAPER.md:164 "the list of selected events is transferred back". */
+int cbm_trigger_fetch_results(cbm_trigger_t* h, uint32_t slot, uint32_t* n_triplets, uint32_t* n_candidates,
+                              uint8_t* accept);
+
+/* Device-resident entry point (PyTorch or any other owner of device memory and streams supplies both):
+ * runs a3-a8 on caller-owned DEVICE arrays on the caller's stream (`stream` is a cudaStream_t passed as void*;
+ * NULL = the legacy default stream).  d_x, d_y: n_hits int32 each, 16-byte aligned, readable up to the next
+ * multiple of 4 elements (over-read by the 128-bit staging copies; contents ignored).  d_off: n_events*L+1
+ * uint32.  Outputs: d_n_triplets[n_events*S] uint32, d_n_candidates[n_events] uint32, d_accept[n_events] uint8.
+ * Asynchronous; the handle's scheduler scratch is reused, so calls on one handle must be stream-ordered.
+ * Requires n_events <= max_events.  Structural errors are reported by cbm_trigger_device_status(). */
+int cbm_trigger_run_device(cbm_trigger_t* h, uint32_t n_events, uint64_t n_hits, const int32_t* d_x,
+                           const int32_t* d_y, const uint32_t* d_off, uint32_t* d_n_triplets,
+                           uint32_t* d_n_candidates, uint8_t* d_accept, void* stream);
+
+/* Synchronises `stream` and fills *stats (HOST) for the last cbm_trigger_run_device call.  Returns
+ * CBM_ERR_RANGE if that run rejected events, CBM_OK otherwise. */
+int cbm_trigger_device_status(cbm_trigger_t* h, void* stream, cbm_trigger_stats_t* stats);
+
+/* Statistics of the last completed run of `slot` (call after fetch_results).  stats: HOST. */
+int cbm_trigger_get_stats(cbm_trigger_t* h, uint32_t slot, cbm_trigger_stats_t* stats);
+
+/* Handle-owned, NUL-terminated message of the last failing call ("" if none).  With h == NULL: the message of
+ * the last failing cbm_trigger_create on this thread. */
+const char* cbm_trigger_last_error(const cbm_trigger_t* h);
+
+/* "cbm-trigger <version> sm_100a" */
+const char* cbm_trigger_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CBM_TRIGGER_H */

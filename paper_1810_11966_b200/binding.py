@@ -1,0 +1,278 @@
+"""Thin ctypes binding of libcbmtrigger.so (include/cbm_trigger.h): argument marshalling only.
+
+Every step of the selection runs in the CUDA kernels behind the C ABI.  There is no CPU fallback:
+if the library has not been built, importing the symbols raises.  The functions carry the names
+of the C entry points; ``Trigger`` is a small convenience wrapper around a handle.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libcbmtrigger.so")
+
+MAX_LAYERS = 24
+N_KERNELS = 4
+KERNEL_NAMES = ("tile_kernel", "team_kernel_M", "team_kernel_H", "team_kernel_G")
+CBM_OK, CBM_ERR_INVALID_ARG, CBM_ERR_RANGE, CBM_ERR_CAPACITY, CBM_ERR_STATE, CBM_ERR_CUDA = 0, -1, -2, -3, -4, -5
+CBM_FLAG_PROFILE, CBM_FLAG_NO_TINY_PATH = 1, 2
+EXPORTS = (
+    "cbm_trigger_create", "cbm_trigger_destroy", "cbm_trigger_host_buffers", "cbm_trigger_upload_events",
+    "cbm_trigger_run", "cbm_trigger_fetch_results", "cbm_trigger_run_device", "cbm_trigger_device_status",
+    "cbm_trigger_get_stats", "cbm_trigger_last_error", "cbm_trigger_version",
+)
+
+
+class Config(ctypes.Structure):
+    _fields_ = [
+        ("struct_size", ctypes.c_uint32),
+        ("n_stations", ctypes.c_uint32),
+        ("layer_z", ctypes.c_int32 * MAX_LAYERS),
+        ("win_in_num", ctypes.c_uint32), ("win_in_den", ctypes.c_uint32),
+        ("win_link_num", ctypes.c_uint32), ("win_link_den", ctypes.c_uint32),
+        ("min_candidates", ctypes.c_uint32),
+        ("max_events", ctypes.c_uint32),
+        ("max_hits", ctypes.c_uint64),
+        ("max_hits_per_layer", ctypes.c_uint32),
+        ("n_slots", ctypes.c_uint32),
+        ("device", ctypes.c_int32),
+        ("slope_range_milli", ctypes.c_uint32),
+        ("tiny_max_layer_hits", ctypes.c_uint32),
+        ("flags", ctypes.c_uint32),
+    ]
+
+
+class Stats(ctypes.Structure):
+    _fields_ = [
+        ("struct_size", ctypes.c_uint32),
+        ("n_events", ctypes.c_uint32),
+        ("n_hits", ctypes.c_uint64),
+        ("n_class", ctypes.c_uint32 * 4),
+        ("n_invalid", ctypes.c_uint32),
+        ("first_invalid", ctypes.c_uint32),
+        ("n_launches", ctypes.c_uint32),
+        ("kernel_ms", ctypes.c_float * N_KERNELS),
+        ("h2d_ms", ctypes.c_float), ("d2h_ms", ctypes.c_float),
+    ]
+
+    def as_dict(self):
+        return {"n_events": self.n_events, "n_hits": self.n_hits, "n_class": list(self.n_class),
+                "n_invalid": self.n_invalid, "first_invalid": self.first_invalid, "n_launches": self.n_launches,
+                "kernel_ms": [float(v) for v in self.kernel_ms], "h2d_ms": float(self.h2d_ms),
+                "d2h_ms": float(self.d2h_ms)}
+
+
+class CbmTriggerError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"cbm_trigger error {code}: {msg}")
+        self.code = code
+
+
+_lib = None
+
+
+def load_library():
+    """dlopen libcbmtrigger.so.  Raises if it is missing: the product has no other path."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError(f"{LIB_PATH} is missing: build it with `python -m paper_1810_11966_b200.build` "
+                               "(nvcc, sm_100a); there is no CPU fallback")
+        lib = ctypes.CDLL(LIB_PATH)
+        vp, u32, u64, i32 = ctypes.c_void_p, ctypes.c_uint32, ctypes.c_uint64, ctypes.c_int
+        lib.cbm_trigger_create.restype = i32
+        lib.cbm_trigger_create.argtypes = [ctypes.POINTER(Config), ctypes.POINTER(vp)]
+        lib.cbm_trigger_destroy.restype = None
+        lib.cbm_trigger_destroy.argtypes = [vp]
+        lib.cbm_trigger_host_buffers.restype = i32
+        lib.cbm_trigger_host_buffers.argtypes = [vp, u32, ctypes.POINTER(vp), ctypes.POINTER(vp), ctypes.POINTER(vp)]
+        lib.cbm_trigger_upload_events.restype = i32
+        lib.cbm_trigger_upload_events.argtypes = [vp, u32, u32, u64, vp, vp, vp]
+        lib.cbm_trigger_run.restype = i32
+        lib.cbm_trigger_run.argtypes = [vp, u32]
+        lib.cbm_trigger_fetch_results.restype = i32
+        lib.cbm_trigger_fetch_results.argtypes = [vp, u32, vp, vp, vp]
+        lib.cbm_trigger_run_device.restype = i32
+        lib.cbm_trigger_run_device.argtypes = [vp, u32, u64, vp, vp, vp, vp, vp, vp, vp]
+        lib.cbm_trigger_device_status.restype = i32
+        lib.cbm_trigger_device_status.argtypes = [vp, vp, ctypes.POINTER(Stats)]
+        lib.cbm_trigger_get_stats.restype = i32
+        lib.cbm_trigger_get_stats.argtypes = [vp, u32, ctypes.POINTER(Stats)]
+        lib.cbm_trigger_last_error.restype = ctypes.c_char_p
+        lib.cbm_trigger_last_error.argtypes = [vp]
+        lib.cbm_trigger_version.restype = ctypes.c_char_p
+        lib.cbm_trigger_version.argtypes = []
+        _lib = lib
+    return _lib
+
+
+def make_config(layer_z, max_events, max_hits, win_in=(1, 100), win_link=(2, 100), min_candidates=2,
+                max_hits_per_layer=4096, n_slots=2, device=0, slope_range_milli=0, tiny_max_layer_hits=0,
+                flags=0) -> Config:
+    c = Config()
+    c.struct_size = ctypes.sizeof(Config)
+    c.n_stations = len(layer_z) // 3
+    for i, z in enumerate(layer_z[:MAX_LAYERS]):
+        c.layer_z[i] = int(z)
+    c.win_in_num, c.win_in_den = win_in
+    c.win_link_num, c.win_link_den = win_link
+    c.min_candidates = min_candidates
+    c.max_events, c.max_hits = int(max_events), int(max_hits)
+    c.max_hits_per_layer = max_hits_per_layer
+    c.n_slots, c.device = n_slots, device
+    c.slope_range_milli, c.tiny_max_layer_hits, c.flags = slope_range_milli, tiny_max_layer_hits, flags
+    return c
+
+
+# ------------------------------------------------------------------ the C entry points, same names
+def cbm_trigger_version() -> str:
+    return load_library().cbm_trigger_version().decode()
+
+
+def cbm_trigger_last_error(handle) -> str:
+    return load_library().cbm_trigger_last_error(handle).decode()
+
+
+def _check(rc, handle):
+    if rc != CBM_OK:
+        raise CbmTriggerError(rc, cbm_trigger_last_error(handle))
+
+
+def cbm_trigger_create(cfg: Config):
+    h = ctypes.c_void_p()
+    rc = load_library().cbm_trigger_create(ctypes.byref(cfg), ctypes.byref(h))
+    _check(rc, None)
+    return h
+
+
+def cbm_trigger_destroy(handle):
+    load_library().cbm_trigger_destroy(handle)
+
+
+def cbm_trigger_host_buffers(handle, slot, max_hits, n_off):
+    """numpy views (no copy) of the slot's pinned staging buffers."""
+    px, py, po = ctypes.c_void_p(), ctypes.c_void_p(), ctypes.c_void_p()
+    _check(load_library().cbm_trigger_host_buffers(handle, slot, ctypes.byref(px), ctypes.byref(py), ctypes.byref(po)),
+           handle)
+    x = np.ctypeslib.as_array(ctypes.cast(px, ctypes.POINTER(ctypes.c_int32)), shape=(max(int(max_hits), 1),))
+    y = np.ctypeslib.as_array(ctypes.cast(py, ctypes.POINTER(ctypes.c_int32)), shape=(max(int(max_hits), 1),))
+    off = np.ctypeslib.as_array(ctypes.cast(po, ctypes.POINTER(ctypes.c_uint32)), shape=(int(n_off),))
+    return x, y, off
+
+
+def _host_ptr(a, dtype):
+    assert isinstance(a, np.ndarray) and a.dtype == dtype and a.flags.c_contiguous, (type(a), getattr(a, "dtype", None))
+    return a.ctypes.data
+
+
+def cbm_trigger_upload_events(handle, slot, n_events, n_hits, x, y, off):
+    _check(load_library().cbm_trigger_upload_events(handle, slot, n_events, n_hits, _host_ptr(x, np.int32),
+                                                    _host_ptr(y, np.int32), _host_ptr(off, np.uint32)), handle)
+
+
+def cbm_trigger_run(handle, slot):
+    _check(load_library().cbm_trigger_run(handle, slot), handle)
+
+
+def cbm_trigger_fetch_results(handle, slot, n_triplets, n_candidates, accept):
+    """Fills the caller's numpy arrays.  Returns the C return code (CBM_OK or CBM_ERR_RANGE), raises on others."""
+    rc = load_library().cbm_trigger_fetch_results(
+        handle, slot, None if n_triplets is None else _host_ptr(n_triplets, np.uint32),
+        _host_ptr(n_candidates, np.uint32), None if accept is None else _host_ptr(accept, np.uint8))
+    if rc not in (CBM_OK, CBM_ERR_RANGE):
+        _check(rc, handle)
+    return rc
+
+
+def cbm_trigger_get_stats(handle, slot) -> Stats:
+    st = Stats()
+    _check(load_library().cbm_trigger_get_stats(handle, slot, ctypes.byref(st)), handle)
+    return st
+
+
+def cbm_trigger_run_device(handle, n_events, n_hits, d_x, d_y, d_off, d_n_triplets, d_n_candidates, d_accept,
+                           stream=0):
+    """d_* are raw device addresses (ints); stream is a cudaStream_t as int."""
+    _check(load_library().cbm_trigger_run_device(handle, n_events, n_hits, d_x, d_y, d_off, d_n_triplets,
+                                                 d_n_candidates, d_accept, stream), handle)
+
+
+def cbm_trigger_device_status(handle, stream=0):
+    st = Stats()
+    rc = load_library().cbm_trigger_device_status(handle, stream, ctypes.byref(st))
+    if rc not in (CBM_OK, CBM_ERR_RANGE):
+        _check(rc, handle)
+    return rc, st
+
+
+# ------------------------------------------------------------------ convenience wrapper
+class Trigger:
+    """Owns one handle.  Host-path: upload/run/fetch on slots.  Device path: run_device on torch tensors."""
+
+    def __init__(self, layer_z, max_events, max_hits, **kw):
+        self.cfg = make_config(layer_z, max_events, max_hits, **kw)
+        self.S = self.cfg.n_stations
+        self.L = 3 * self.S
+        self.handle = cbm_trigger_create(self.cfg)
+
+    def close(self):
+        if self.handle is not None:
+            cbm_trigger_destroy(self.handle)
+            self.handle = None
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
+        self.close()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def host_buffers(self, slot):
+        return cbm_trigger_host_buffers(self.handle, slot, self.cfg.max_hits, self.cfg.max_events * self.L + 1)
+
+    def upload_events(self, slot, x, y, off, n_events=None, n_hits=None):
+        n_events = (off.size - 1) // self.L if n_events is None else n_events
+        n_hits = int(off[n_events * self.L]) if n_hits is None else n_hits
+        cbm_trigger_upload_events(self.handle, slot, n_events, n_hits, x, y, off)
+        return n_events, n_hits
+
+    def run(self, slot):
+        cbm_trigger_run(self.handle, slot)
+
+    def fetch_results(self, slot, n_events, out=None, check=True):
+        if out is None:
+            out = (np.empty((n_events, self.S), dtype=np.uint32), np.empty(n_events, dtype=np.uint32),
+                   np.empty(n_events, dtype=np.uint8))
+        rc = cbm_trigger_fetch_results(self.handle, slot, out[0], out[1], out[2])
+        if check and rc != CBM_OK:
+            raise CbmTriggerError(rc, cbm_trigger_last_error(self.handle))
+        return out if check else (out, rc)
+
+    def stats(self, slot) -> Stats:
+        return cbm_trigger_get_stats(self.handle, slot)
+
+    def select(self, x, y, off, slot=0):
+        """upload + run + fetch of one host batch (numpy arrays)."""
+        n_events, _ = self.upload_events(slot, x, y, off)
+        self.run(slot)
+        return self.fetch_results(slot, n_events)
+
+    def run_device(self, n_events, n_hits, d_x, d_y, d_off, d_nt, d_nc, d_ac, stream=None):
+        """torch CUDA tensors in, torch CUDA tensors out (PyTorch supplies memory and the stream)."""
+        import torch
+        st = torch.cuda.current_stream().cuda_stream if stream is None else stream
+        cbm_trigger_run_device(self.handle, n_events, n_hits, d_x.data_ptr(), d_y.data_ptr(), d_off.data_ptr(),
+                               d_nt.data_ptr(), d_nc.data_ptr(), d_ac.data_ptr(), st)
+
+    def device_status(self, stream=None):
+        import torch
+        st = torch.cuda.current_stream().cuda_stream if stream is None else stream
+        return cbm_trigger_device_status(self.handle, st)

@@ -1,0 +1,542 @@
+// cbm_trigger.cu -- host side of libcbmtrigger.so: the C ABI of include/cbm_trigger.h.
+//
+// Owns the slots (pinned host staging, device arrays, result buffers), the three streams of the
+// H2D | kernels | D2H software pipeline ("it can be hidden by performing computation and
+// transfer in parallel") and the launch sequence of the kernels in kernels.cuh.  No CPU fallback exists:
+// without a CUDA device cbm_trigger_create fails with CBM_ERR_CUDA.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <string>
+
+#include "../../include/cbm_trigger.h"
+#include "kernels.cuh"
+
+namespace {
+
+using namespace cbm;
+
+// team classes: warps per team, fullest layer admitted, cells per binned layer
+constexpr int kWM = 1, kCapM = 128, kNcM = 576;
+constexpr int kWH = 4, kCapH = 512, kNcH = 2304;
+constexpr int kWG = 16, kCapG = 4096, kNcG = 2304;
+using SmemM = TeamSmem<kWM, kCapM, kNcM>;
+using SmemH = TeamSmem<kWH, kCapH, kNcH>;
+using SmemG = TeamSmem<kWG, kCapG, kNcG>;
+
+enum SlotState { kEmpty = 0, kUploaded = 1, kRunning = 2 };
+
+struct Scratch {
+  Ctrl* d_ctrl = nullptr;
+  uint32_t* d_list[kNumTeamClasses] = {nullptr, nullptr, nullptr};
+};
+
+struct ProfEvents {
+  cudaEvent_t k[CBM_TRIGGER_N_KERNELS + 1] = {};
+  cudaEvent_t h2d[2] = {}, d2h[2] = {};
+  bool valid = false;
+};
+
+struct Slot {
+  int32_t *h_x = nullptr, *h_y = nullptr;
+  uint32_t* h_off = nullptr;
+  int32_t *d_x = nullptr, *d_y = nullptr;
+  uint32_t* d_off = nullptr;
+  uint32_t *d_nt = nullptr, *d_nc = nullptr;
+  uint8_t* d_ac = nullptr;
+  uint32_t *h_nt = nullptr, *h_nc = nullptr;
+  uint8_t* h_ac = nullptr;
+  Ctrl* h_ctrl = nullptr;
+  Scratch scr;
+  ProfEvents prof;
+  cudaEvent_t ev_h2d = nullptr, ev_run = nullptr, ev_d2h = nullptr;
+  int state = kEmpty;
+  uint32_t n_events = 0;
+  uint64_t n_hits = 0;
+  cbm_trigger_stats_t stats = {};
+};
+
+}  // namespace
+
+struct cbm_trigger {
+  cbm_trigger_config_t cfg;
+  Params p;
+  int n_sm = 0;
+  int grid[kNumTeamClasses] = {0, 0, 0};
+  Slot slot[CBM_TRIGGER_MAX_SLOTS];
+  Scratch dev_scr;          // scratch of cbm_trigger_run_device
+  Ctrl* h_dev_ctrl = nullptr;
+  ProfEvents dev_prof;
+  uint32_t dev_n_events = 0;
+  uint64_t dev_n_hits = 0;
+  cudaStream_t st_h2d = nullptr, st_run = nullptr, st_d2h = nullptr;
+  std::string err;
+};
+
+namespace {
+
+thread_local std::string g_create_err;
+
+int fail(cbm_trigger* h, int code, const char* fmt, ...) {
+  char buf[512];
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(buf, sizeof(buf), fmt, ap);
+  va_end(ap);
+  if (h) h->err = buf; else g_create_err = buf;
+  return code;
+}
+
+#define CBM_CUDA(h, expr)                                                                       \
+  do {                                                                                          \
+    cudaError_t e_ = (expr);                                                                    \
+    if (e_ != cudaSuccess) return fail(h, CBM_ERR_CUDA, "%s: %s", #expr, cudaGetErrorString(e_)); \
+  } while (0)
+
+// ---------------------------------------------------------------------------------------------- parameters
+int build_params(const cbm_trigger_config_t& c, Params& p, std::string& why) {
+  memset(&p, 0, sizeof(p));
+  if (c.n_stations < 1 || c.n_stations > CBM_TRIGGER_MAX_STATIONS) { why = "n_stations must be 1..8"; return CBM_ERR_INVALID_ARG; }
+  p.S = c.n_stations;
+  p.L = 3 * c.n_stations;
+  for (uint32_t l = 0; l < p.L; ++l) {
+    const int32_t z = c.layer_z[l];
+    if (z <= 0 || z > (1 << 23)) { why = "layer_z must be in (0, 2^23]"; return CBM_ERR_INVALID_ARG; }
+    if (l && z <= c.layer_z[l - 1]) { why = "layer_z must be strictly increasing"; return CBM_ERR_INVALID_ARG; }
+    p.z[l] = z;
+  }
+  if (c.win_in_den == 0 || c.win_in_den > 4096 || c.win_in_num > c.win_in_den ||
+      c.win_link_den == 0 || c.win_link_den > 4096 || c.win_link_num > c.win_link_den) {
+    why = "windows need 0 < den <= 4096 and num <= den";
+    return CBM_ERR_INVALID_ARG;
+  }
+  if (c.max_hits_per_layer < 1 || c.max_hits_per_layer > CBM_TRIGGER_MAX_HITS_PER_LAYER) {
+    why = "max_hits_per_layer must be 1..4096";
+    return CBM_ERR_INVALID_ARG;
+  }
+  if (c.n_slots > CBM_TRIGGER_MAX_SLOTS) { why = "n_slots must be 0..4"; return CBM_ERR_INVALID_ARG; }
+  if (c.max_events == 0) { why = "max_events must be > 0"; return CBM_ERR_INVALID_ARG; }
+  if (c.max_hits >= (1ull << 32)) { why = "max_hits must be < 2^32"; return CBM_ERR_INVALID_ARG; }
+  if ((uint64_t)c.max_events * p.L + 1 >= (1ull << 32)) { why = "max_events * layers must be < 2^32"; return CBM_ERR_INVALID_ARG; }
+  if (c.tiny_max_layer_hits > kTinyMaxLayerLimit) { why = "tiny_max_layer_hits must be <= 32"; return CBM_ERR_INVALID_ARG; }
+  if (c.device < 0) { why = "device must be >= 0"; return CBM_ERR_INVALID_ARG; }
+
+  // R4: per-layer-pair integer thresholds T_AB = floor(a*z_A*z_B / b); a*z_A*z_B <= 2^12 * 2^46
+  for (uint32_t s = 0; s < p.S; ++s) {
+    const int64_t z0 = p.z[3 * s], z1 = p.z[3 * s + 1], z2 = p.z[3 * s + 2];
+    const int64_t a = c.win_in_num, b = c.win_in_den;
+    p.thr_in[s][0] = a * z0 * z1 / b;
+    p.thr_in[s][1] = a * z0 * z2 / b;
+    p.thr_in[s][2] = a * z1 * z2 / b;
+    if (s) {
+      const int64_t zA = p.z[3 * (s - 1) + 1];
+      p.thr_link[s] = (int64_t)c.win_link_num * zA * z1 / (int64_t)c.win_link_den;
+    }
+  }
+  p.min_candidates = c.min_candidates;
+  p.max_hits_per_layer = c.max_hits_per_layer;
+  const bool tiny_on = !(c.flags & CBM_FLAG_NO_TINY_PATH);
+  p.tiny_max_layer = c.tiny_max_layer_hits ? c.tiny_max_layer_hits : 24;
+  p.tiny_max_total = tiny_on ? kTinyMaxTotal : 0;
+  p.cls_max[kClsM] = kCapM; p.cls_max[kClsH] = kCapH; p.cls_max[kClsG] = kCapG;
+
+  // Slope keys: key = floor(x*M_l/2^32), M_l = round(2^32*K/z_l) < 2^31.
+  // For any int32 x: |x*M_l/2^32 - K*x/z_l| <= 2^31 * 0.5/2^32 = 0.25, floor loses < 1  =>  |key - K*x/z_l| < 1.25.
+  // Two hits with |x_h/z_A - x_g/z_B| <= w therefore have |key_h - key_g| < w*K + 2.5 <= R := ceil(w*K) + 3.
+  const double w = (double)c.win_in_num / (double)c.win_in_den;
+  const double smax = (c.slope_range_milli ? c.slope_range_milli : 400) / 1000.0;
+  const double Kmax = 0.499 * (double)p.z[0];
+  double cell = std::max(2.0 * w * 1.05, 2.0 * smax / 44.0);
+  bool ok = false;
+  int sh = 0;
+  double K = 0;
+  int R = 0;
+  for (int it = 0; it < 64 && !ok; ++it, cell *= 1.25) {
+    const double lim = cell * Kmax;
+    if (lim < 4.0) break;
+    sh = (int)std::floor(std::log2(lim));
+    if (sh > 14) sh = 14;
+    K = std::ldexp(1.0, sh) / cell;
+    R = (int)std::ceil(w * K) + 3;
+    ok = 2 * R <= (1 << sh);
+  }
+  if (!ok) {  // geometry too fine for the key resolution: one bin per layer (still exact, just slower)
+    K = Kmax; sh = 30; R = 0;
+    for (int c3 = 0; c3 < kNumTeamClasses; ++c3) { p.cls_shift[c3] = 30; p.cls_nb[c3] = 1; }
+    p.key_min = 0;
+  } else {
+    const int half = (int)std::ceil(smax * K);
+    p.key_min = -half;
+    int shH = sh;
+    while (((2 * half) >> shH) + 1 > 48) ++shH;
+    p.cls_shift[kClsH] = p.cls_shift[kClsG] = shH;
+    p.cls_nb[kClsH] = p.cls_nb[kClsG] = (uint32_t)(((2 * half) >> shH) + 1);
+    p.cls_shift[kClsM] = shH + 1;
+    p.cls_nb[kClsM] = (uint32_t)(((2 * half) >> (shH + 1)) + 1);
+  }
+  p.key_R = R;
+  for (uint32_t l = 0; l < p.L; ++l) {
+    const double m = std::ldexp(K, 32) / (double)p.z[l];
+    const long long mi = llround(m);
+    if (mi < 0 || mi > 0x7FFFFFFFll) { why = "internal: key multiplier out of range"; return CBM_ERR_INVALID_ARG; }
+    p.key_mul[l] = (int32_t)mi;
+  }
+  if (p.cls_nb[kClsM] * p.cls_nb[kClsM] > (uint32_t)kNcM || p.cls_nb[kClsH] * p.cls_nb[kClsH] > (uint32_t)kNcH) {
+    why = "internal: bin grid too large";
+    return CBM_ERR_INVALID_ARG;
+  }
+  return CBM_OK;
+}
+
+// ---------------------------------------------------------------------------------------------- allocation
+int alloc_scratch(cbm_trigger* h, Scratch& s) {
+  CBM_CUDA(h, cudaMalloc(&s.d_ctrl, sizeof(Ctrl)));
+  for (int c = 0; c < kNumTeamClasses; ++c) CBM_CUDA(h, cudaMalloc(&s.d_list[c], (size_t)h->cfg.max_events * sizeof(uint32_t)));
+  return CBM_OK;
+}
+void free_scratch(Scratch& s) {
+  cudaFree(s.d_ctrl);
+  for (int c = 0; c < kNumTeamClasses; ++c) cudaFree(s.d_list[c]);
+  s = Scratch();
+}
+int make_prof(cbm_trigger* h, ProfEvents& pe) {
+  for (auto& e : pe.k) CBM_CUDA(h, cudaEventCreate(&e));
+  for (auto& e : pe.h2d) CBM_CUDA(h, cudaEventCreate(&e));
+  for (auto& e : pe.d2h) CBM_CUDA(h, cudaEventCreate(&e));
+  return CBM_OK;
+}
+void free_prof(ProfEvents& pe) {
+  for (auto& e : pe.k) if (e) cudaEventDestroy(e);
+  for (auto& e : pe.h2d) if (e) cudaEventDestroy(e);
+  for (auto& e : pe.d2h) if (e) cudaEventDestroy(e);
+  pe = ProfEvents();
+}
+
+int alloc_slot(cbm_trigger* h, Slot& s) {
+  const cbm_trigger_config_t& c = h->cfg;
+  const size_t nh = (size_t)((c.max_hits + 3) & ~3ull) + 4;  // 16-byte tail padding for the bulk copies
+  const size_t noff = (size_t)c.max_events * h->p.L + 1;
+  const size_t ne = c.max_events, S = h->p.S;
+  CBM_CUDA(h, cudaHostAlloc(&s.h_x, nh * 4, cudaHostAllocDefault));
+  CBM_CUDA(h, cudaHostAlloc(&s.h_y, nh * 4, cudaHostAllocDefault));
+  CBM_CUDA(h, cudaHostAlloc(&s.h_off, noff * 4, cudaHostAllocDefault));
+  CBM_CUDA(h, cudaMalloc(&s.d_x, nh * 4));
+  CBM_CUDA(h, cudaMalloc(&s.d_y, nh * 4));
+  CBM_CUDA(h, cudaMalloc(&s.d_off, noff * 4));
+  CBM_CUDA(h, cudaMalloc(&s.d_nt, ne * S * 4));
+  CBM_CUDA(h, cudaMalloc(&s.d_nc, ne * 4));
+  CBM_CUDA(h, cudaMalloc(&s.d_ac, ne));
+  CBM_CUDA(h, cudaHostAlloc(&s.h_nt, ne * S * 4, cudaHostAllocDefault));
+  CBM_CUDA(h, cudaHostAlloc(&s.h_nc, ne * 4, cudaHostAllocDefault));
+  CBM_CUDA(h, cudaHostAlloc(&s.h_ac, ne, cudaHostAllocDefault));
+  CBM_CUDA(h, cudaHostAlloc(&s.h_ctrl, sizeof(Ctrl), cudaHostAllocDefault));
+  CBM_CUDA(h, cudaMemset(s.d_x + (nh - 8), 0, 32));
+  CBM_CUDA(h, cudaMemset(s.d_y + (nh - 8), 0, 32));
+  int rc = alloc_scratch(h, s.scr);
+  if (rc) return rc;
+  CBM_CUDA(h, cudaEventCreateWithFlags(&s.ev_h2d, cudaEventDisableTiming));
+  CBM_CUDA(h, cudaEventCreateWithFlags(&s.ev_run, cudaEventDisableTiming));
+  CBM_CUDA(h, cudaEventCreateWithFlags(&s.ev_d2h, cudaEventDisableTiming));
+  if (c.flags & CBM_FLAG_PROFILE) { rc = make_prof(h, s.prof); if (rc) return rc; }
+  return CBM_OK;
+}
+void free_slot(Slot& s) {
+  cudaFreeHost(s.h_x); cudaFreeHost(s.h_y); cudaFreeHost(s.h_off);
+  cudaFree(s.d_x); cudaFree(s.d_y); cudaFree(s.d_off);
+  cudaFree(s.d_nt); cudaFree(s.d_nc); cudaFree(s.d_ac);
+  cudaFreeHost(s.h_nt); cudaFreeHost(s.h_nc); cudaFreeHost(s.h_ac); cudaFreeHost(s.h_ctrl);
+  free_scratch(s.scr);
+  free_prof(s.prof);
+  if (s.ev_h2d) cudaEventDestroy(s.ev_h2d);
+  if (s.ev_run) cudaEventDestroy(s.ev_run);
+  if (s.ev_d2h) cudaEventDestroy(s.ev_d2h);
+  s = Slot();
+}
+
+// ---------------------------------------------------------------------------------------------- launches
+// a3..a8 on one stream.  Returns the number of kernels launched (0 on an empty batch), < 0 on error.
+int launch_selection(cbm_trigger* h, const Scratch& scr, const int32_t* d_x, const int32_t* d_y, const uint32_t* d_off,
+                     uint32_t n_events, uint64_t n_hits, uint32_t* d_nt, uint32_t* d_nc, uint8_t* d_ac,
+                     cudaStream_t st, ProfEvents* prof) {
+  const Params& p = h->p;
+  CBM_CUDA(h, cudaMemsetAsync(scr.d_ctrl, 0, sizeof(Ctrl), st));
+  if (prof) prof->valid = false;
+  if (n_events == 0) return 0;
+  if (prof) CBM_CUDA(h, cudaEventRecord(prof->k[0], st));
+  const uint32_t n_tiles = (n_events + kTileEvents - 1) / kTileEvents;
+  tile_kernel<<<n_tiles, kTileEvents * p.S, 0, st>>>(p, d_x, d_y, d_off, n_events, (uint32_t)n_hits, d_nt, d_nc, d_ac,
+                                                     scr.d_ctrl, scr.d_list[kClsM], scr.d_list[kClsH], scr.d_list[kClsG]);
+  if (prof) CBM_CUDA(h, cudaEventRecord(prof->k[1], st));
+  team_kernel<kWM, kCapM, kNcM, kClsM><<<h->grid[kClsM], 32 * kWM, sizeof(SmemM), st>>>(
+      p, d_x, d_y, d_off, d_nt, d_nc, d_ac, scr.d_ctrl, scr.d_list[kClsM]);
+  if (prof) CBM_CUDA(h, cudaEventRecord(prof->k[2], st));
+  team_kernel<kWH, kCapH, kNcH, kClsH><<<h->grid[kClsH], 32 * kWH, sizeof(SmemH), st>>>(
+      p, d_x, d_y, d_off, d_nt, d_nc, d_ac, scr.d_ctrl, scr.d_list[kClsH]);
+  if (prof) CBM_CUDA(h, cudaEventRecord(prof->k[3], st));
+  team_kernel<kWG, kCapG, kNcG, kClsG><<<h->grid[kClsG], 32 * kWG, sizeof(SmemG), st>>>(
+      p, d_x, d_y, d_off, d_nt, d_nc, d_ac, scr.d_ctrl, scr.d_list[kClsG]);
+  if (prof) { CBM_CUDA(h, cudaEventRecord(prof->k[4], st)); prof->valid = true; }
+  CBM_CUDA(h, cudaGetLastError());
+  return 4;
+}
+
+void fill_stats(cbm_trigger_stats_t& st, const Ctrl& c, uint32_t n_events, uint64_t n_hits, uint32_t n_launches) {
+  memset(&st, 0, sizeof(st));
+  st.struct_size = sizeof(st);
+  st.n_events = n_events;
+  st.n_hits = n_hits;
+  st.n_class[1] = c.count[kClsM]; st.n_class[2] = c.count[kClsH]; st.n_class[3] = c.count[kClsG];
+  st.n_invalid = c.n_invalid;
+  st.first_invalid = c.first_invalid_inv ? ~c.first_invalid_inv : 0xFFFFFFFFu;
+  // escalated events were first handled by the tile kernel, then redone by team_M
+  st.n_class[0] = n_events - (c.count[kClsM] - c.n_escalated) - c.count[kClsH] - c.count[kClsG] - c.n_invalid;
+  st.n_launches = n_launches;
+}
+
+void fill_prof(cbm_trigger_stats_t& st, ProfEvents& pe, bool copies) {
+  if (!pe.valid) return;
+  for (int k = 0; k < CBM_TRIGGER_N_KERNELS; ++k) {
+    float ms = 0;
+    if (cudaEventElapsedTime(&ms, pe.k[k], pe.k[k + 1]) == cudaSuccess) st.kernel_ms[k] = ms;
+  }
+  if (copies) {
+    float ms = 0;
+    if (cudaEventElapsedTime(&ms, pe.h2d[0], pe.h2d[1]) == cudaSuccess) st.h2d_ms = ms;
+    if (cudaEventElapsedTime(&ms, pe.d2h[0], pe.d2h[1]) == cudaSuccess) st.d2h_ms = ms;
+  }
+}
+
+template <class K>
+int occupancy_grid(cbm_trigger* h, K kernel, int threads, size_t smem, int* grid) {
+  CBM_CUDA(h, cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  int per_sm = 0;
+  CBM_CUDA(h, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, threads, smem));
+  if (per_sm < 1) return fail(h, CBM_ERR_CUDA, "a team kernel does not fit on this device");
+  *grid = per_sm * h->n_sm;
+  return CBM_OK;
+}
+
+}  // namespace
+
+// ================================================================================================ C ABI
+extern "C" {
+
+const char* cbm_trigger_version(void) { return "cbm-trigger 0.1 sm_100a"; }
+
+const char* cbm_trigger_last_error(const cbm_trigger_t* h) { return h ? h->err.c_str() : g_create_err.c_str(); }
+
+int cbm_trigger_create(const cbm_trigger_config_t* cfg, cbm_trigger_t** out) {
+  if (!cfg || !out) return fail(nullptr, CBM_ERR_INVALID_ARG, "cfg and out must not be NULL");
+  if (cfg->struct_size != sizeof(cbm_trigger_config_t))
+    return fail(nullptr, CBM_ERR_INVALID_ARG, "struct_size %u != %zu", cfg->struct_size, sizeof(cbm_trigger_config_t));
+  Params p;
+  std::string why;
+  int rc = build_params(*cfg, p, why);
+  if (rc) return fail(nullptr, rc, "%s", why.c_str());
+
+  cbm_trigger* h = new (std::nothrow) cbm_trigger();
+  if (!h) return fail(nullptr, CBM_ERR_CUDA, "out of host memory");
+  h->cfg = *cfg;
+  h->p = p;
+  auto bail = [&](int code) {
+    g_create_err = h->err;
+    cbm_trigger_destroy(h);
+    return code;
+  };
+  int n_dev = 0;
+  cudaError_t e = cudaGetDeviceCount(&n_dev);
+  if (e != cudaSuccess || n_dev == 0) {
+    fail(h, CBM_ERR_CUDA, "no CUDA device: %s (there is no CPU fallback)", e != cudaSuccess ? cudaGetErrorString(e) : "count is 0");
+    return bail(CBM_ERR_CUDA);
+  }
+  if (cfg->device >= n_dev) { fail(h, CBM_ERR_INVALID_ARG, "device %d of %d", cfg->device, n_dev); return bail(CBM_ERR_INVALID_ARG); }
+#define CREATE_TRY(call) do { int rc_ = (call); if (rc_) return bail(rc_); } while (0)
+#define CREATE_CUDA(expr) do { cudaError_t e_ = (expr); if (e_ != cudaSuccess) { fail(h, CBM_ERR_CUDA, "%s: %s", #expr, cudaGetErrorString(e_)); return bail(CBM_ERR_CUDA); } } while (0)
+  CREATE_CUDA(cudaSetDevice(cfg->device));
+  cudaDeviceProp prop;
+  CREATE_CUDA(cudaGetDeviceProperties(&prop, cfg->device));
+  if (prop.major < 10) { fail(h, CBM_ERR_CUDA, "device is sm_%d%d; this library holds sm_100a code only", prop.major, prop.minor); return bail(CBM_ERR_CUDA); }
+  h->n_sm = prop.multiProcessorCount;
+  CREATE_TRY(occupancy_grid(h, team_kernel<kWM, kCapM, kNcM, kClsM>, 32 * kWM, sizeof(SmemM), &h->grid[kClsM]));
+  CREATE_TRY(occupancy_grid(h, team_kernel<kWH, kCapH, kNcH, kClsH>, 32 * kWH, sizeof(SmemH), &h->grid[kClsH]));
+  CREATE_TRY(occupancy_grid(h, team_kernel<kWG, kCapG, kNcG, kClsG>, 32 * kWG, sizeof(SmemG), &h->grid[kClsG]));
+  CREATE_CUDA(cudaStreamCreateWithFlags(&h->st_h2d, cudaStreamNonBlocking));
+  CREATE_CUDA(cudaStreamCreateWithFlags(&h->st_run, cudaStreamNonBlocking));
+  CREATE_CUDA(cudaStreamCreateWithFlags(&h->st_d2h, cudaStreamNonBlocking));
+  CREATE_TRY(alloc_scratch(h, h->dev_scr));
+  CREATE_CUDA(cudaHostAlloc(&h->h_dev_ctrl, sizeof(Ctrl), cudaHostAllocDefault));
+  if (cfg->flags & CBM_FLAG_PROFILE) CREATE_TRY(make_prof(h, h->dev_prof));
+  for (uint32_t i = 0; i < cfg->n_slots; ++i) CREATE_TRY(alloc_slot(h, h->slot[i]));
+#undef CREATE_TRY
+#undef CREATE_CUDA
+  *out = h;
+  return CBM_OK;
+}
+
+void cbm_trigger_destroy(cbm_trigger_t* h) {
+  if (!h) return;
+  if (h->st_h2d || h->st_run || h->st_d2h) {
+    cudaSetDevice(h->cfg.device);
+    if (h->st_h2d) cudaStreamSynchronize(h->st_h2d);
+    if (h->st_run) cudaStreamSynchronize(h->st_run);
+    if (h->st_d2h) cudaStreamSynchronize(h->st_d2h);
+  }
+  for (auto& s : h->slot) free_slot(s);
+  free_scratch(h->dev_scr);
+  free_prof(h->dev_prof);
+  if (h->h_dev_ctrl) cudaFreeHost(h->h_dev_ctrl);
+  if (h->st_h2d) cudaStreamDestroy(h->st_h2d);
+  if (h->st_run) cudaStreamDestroy(h->st_run);
+  if (h->st_d2h) cudaStreamDestroy(h->st_d2h);
+  delete h;
+}
+
+static int check_slot(cbm_trigger_t* h, uint32_t slot) {
+  if (!h) return CBM_ERR_INVALID_ARG;
+  if (slot >= h->cfg.n_slots) return fail(h, CBM_ERR_STATE, "slot %u of %u", slot, h->cfg.n_slots);
+  return CBM_OK;
+}
+
+int cbm_trigger_host_buffers(cbm_trigger_t* h, uint32_t slot, int32_t** x, int32_t** y, uint32_t** off) {
+  int rc = check_slot(h, slot);
+  if (rc) return rc;
+  if (!x || !y || !off) return fail(h, CBM_ERR_INVALID_ARG, "x, y, off must not be NULL");
+  *x = h->slot[slot].h_x; *y = h->slot[slot].h_y; *off = h->slot[slot].h_off;
+  return CBM_OK;
+}
+
+int cbm_trigger_upload_events(cbm_trigger_t* h, uint32_t slot, uint32_t n_events, uint64_t n_hits, const int32_t* x,
+                              const int32_t* y, const uint32_t* off) {
+  int rc = check_slot(h, slot);
+  if (rc) return rc;
+  Slot& s = h->slot[slot];
+  if (!off || (n_hits && (!x || !y))) return fail(h, CBM_ERR_INVALID_ARG, "x, y, off must not be NULL");
+  if (n_events > h->cfg.max_events) return fail(h, CBM_ERR_CAPACITY, "n_events %u > max_events %u", n_events, h->cfg.max_events);
+  if (n_hits > h->cfg.max_hits) return fail(h, CBM_ERR_CAPACITY, "n_hits %llu > max_hits %llu", (unsigned long long)n_hits, (unsigned long long)h->cfg.max_hits);
+  if (s.state == kRunning) return fail(h, CBM_ERR_STATE, "slot %u holds unfetched results", slot);
+  const size_t n_off = (size_t)n_events * h->p.L + 1;
+  if (off[0] != 0 || off[n_off - 1] != n_hits)
+    return fail(h, CBM_ERR_RANGE, "off[0] must be 0 and off[n_events*L] must equal n_hits");
+  CBM_CUDA(h, cudaSetDevice(h->cfg.device));
+  // the staging buffers may still be the source of the slot's previous H2D
+  CBM_CUDA(h, cudaEventSynchronize(s.ev_h2d));
+  if (x != s.h_x && n_hits) memcpy(s.h_x, x, n_hits * 4);
+  if (y != s.h_y && n_hits) memcpy(s.h_y, y, n_hits * 4);
+  if (off != s.h_off) memcpy(s.h_off, off, n_off * 4);
+  // the device arrays may still be read by the slot's previous kernels
+  CBM_CUDA(h, cudaStreamWaitEvent(h->st_h2d, s.ev_run, 0));
+  const bool prof = h->cfg.flags & CBM_FLAG_PROFILE;
+  if (prof) CBM_CUDA(h, cudaEventRecord(s.prof.h2d[0], h->st_h2d));
+  if (n_hits) {
+    CBM_CUDA(h, cudaMemcpyAsync(s.d_x, s.h_x, n_hits * 4, cudaMemcpyHostToDevice, h->st_h2d));
+    CBM_CUDA(h, cudaMemcpyAsync(s.d_y, s.h_y, n_hits * 4, cudaMemcpyHostToDevice, h->st_h2d));
+  }
+  CBM_CUDA(h, cudaMemcpyAsync(s.d_off, s.h_off, n_off * 4, cudaMemcpyHostToDevice, h->st_h2d));
+  if (prof) CBM_CUDA(h, cudaEventRecord(s.prof.h2d[1], h->st_h2d));
+  CBM_CUDA(h, cudaEventRecord(s.ev_h2d, h->st_h2d));
+  s.n_events = n_events;
+  s.n_hits = n_hits;
+  s.state = kUploaded;
+  return CBM_OK;
+}
+
+int cbm_trigger_run(cbm_trigger_t* h, uint32_t slot) {
+  int rc = check_slot(h, slot);
+  if (rc) return rc;
+  Slot& s = h->slot[slot];
+  if (s.state != kUploaded) return fail(h, CBM_ERR_STATE, "slot %u: run needs a preceding upload_events", slot);
+  CBM_CUDA(h, cudaSetDevice(h->cfg.device));
+  const bool prof = h->cfg.flags & CBM_FLAG_PROFILE;
+  CBM_CUDA(h, cudaStreamWaitEvent(h->st_run, s.ev_h2d, 0));
+  CBM_CUDA(h, cudaStreamWaitEvent(h->st_run, s.ev_d2h, 0));  // previous results of this slot must have left
+  const int nl = launch_selection(h, s.scr, s.d_x, s.d_y, s.d_off, s.n_events, s.n_hits, s.d_nt, s.d_nc, s.d_ac,
+                                  h->st_run, prof ? &s.prof : nullptr);
+  if (nl < 0) return nl;
+  CBM_CUDA(h, cudaEventRecord(s.ev_run, h->st_run));
+  CBM_CUDA(h, cudaStreamWaitEvent(h->st_d2h, s.ev_run, 0));
+  if (prof) CBM_CUDA(h, cudaEventRecord(s.prof.d2h[0], h->st_d2h));
+  const size_t ne = s.n_events, S = h->p.S;
+  if (ne) {
+    CBM_CUDA(h, cudaMemcpyAsync(s.h_nt, s.d_nt, ne * S * 4, cudaMemcpyDeviceToHost, h->st_d2h));
+    CBM_CUDA(h, cudaMemcpyAsync(s.h_nc, s.d_nc, ne * 4, cudaMemcpyDeviceToHost, h->st_d2h));
+    CBM_CUDA(h, cudaMemcpyAsync(s.h_ac, s.d_ac, ne, cudaMemcpyDeviceToHost, h->st_d2h));
+  }
+  CBM_CUDA(h, cudaMemcpyAsync(s.h_ctrl, s.scr.d_ctrl, sizeof(Ctrl), cudaMemcpyDeviceToHost, h->st_d2h));
+  if (prof) CBM_CUDA(h, cudaEventRecord(s.prof.d2h[1], h->st_d2h));
+  CBM_CUDA(h, cudaEventRecord(s.ev_d2h, h->st_d2h));
+  s.stats.n_launches = (uint32_t)nl;
+  s.state = kRunning;
+  return CBM_OK;
+}
+
+int cbm_trigger_fetch_results(cbm_trigger_t* h, uint32_t slot, uint32_t* n_triplets, uint32_t* n_candidates,
+                              uint8_t* accept) {
+  int rc = check_slot(h, slot);
+  if (rc) return rc;
+  Slot& s = h->slot[slot];
+  if (s.state != kRunning) return fail(h, CBM_ERR_STATE, "slot %u: fetch_results needs a preceding run", slot);
+  if (!n_candidates && s.n_events) return fail(h, CBM_ERR_INVALID_ARG, "n_candidates must not be NULL");
+  CBM_CUDA(h, cudaSetDevice(h->cfg.device));
+  CBM_CUDA(h, cudaEventSynchronize(s.ev_d2h));
+  const size_t ne = s.n_events, S = h->p.S;
+  if (ne) {
+    if (n_triplets) memcpy(n_triplets, s.h_nt, ne * S * 4);
+    memcpy(n_candidates, s.h_nc, ne * 4);
+    if (accept) memcpy(accept, s.h_ac, ne);
+  }
+  const uint32_t nl = s.stats.n_launches;
+  fill_stats(s.stats, *s.h_ctrl, s.n_events, s.n_hits, nl);
+  if (h->cfg.flags & CBM_FLAG_PROFILE) fill_prof(s.stats, s.prof, true);
+  s.state = kEmpty;
+  if (s.stats.n_invalid)
+    return fail(h, CBM_ERR_RANGE, "%u event(s) rejected on the device (offsets not monotone, beyond n_hits, or a layer above max_hits_per_layer); first: event %u",
+                s.stats.n_invalid, s.stats.first_invalid);
+  return CBM_OK;
+}
+
+int cbm_trigger_get_stats(cbm_trigger_t* h, uint32_t slot, cbm_trigger_stats_t* stats) {
+  int rc = check_slot(h, slot);
+  if (rc) return rc;
+  if (!stats) return fail(h, CBM_ERR_INVALID_ARG, "stats must not be NULL");
+  *stats = h->slot[slot].stats;
+  stats->struct_size = sizeof(*stats);
+  return CBM_OK;
+}
+
+int cbm_trigger_run_device(cbm_trigger_t* h, uint32_t n_events, uint64_t n_hits, const int32_t* d_x, const int32_t* d_y,
+                           const uint32_t* d_off, uint32_t* d_n_triplets, uint32_t* d_n_candidates, uint8_t* d_accept,
+                           void* stream) {
+  if (!h) return CBM_ERR_INVALID_ARG;
+  if (n_events > h->cfg.max_events) return fail(h, CBM_ERR_CAPACITY, "n_events %u > max_events %u", n_events, h->cfg.max_events);
+  if (n_hits >= (1ull << 32)) return fail(h, CBM_ERR_CAPACITY, "n_hits must be < 2^32");
+  if (n_events && (!d_off || !d_n_triplets || !d_n_candidates || !d_accept || (n_hits && (!d_x || !d_y))))
+    return fail(h, CBM_ERR_INVALID_ARG, "device pointers must not be NULL");
+  if (((uintptr_t)d_x | (uintptr_t)d_y) & 15) return fail(h, CBM_ERR_INVALID_ARG, "d_x and d_y must be 16-byte aligned");
+  CBM_CUDA(h, cudaSetDevice(h->cfg.device));
+  const int nl = launch_selection(h, h->dev_scr, d_x, d_y, d_off, n_events, n_hits, d_n_triplets, d_n_candidates,
+                                  d_accept, (cudaStream_t)stream, (h->cfg.flags & CBM_FLAG_PROFILE) ? &h->dev_prof : nullptr);
+  if (nl < 0) return nl;
+  h->dev_n_events = n_events;
+  h->dev_n_hits = n_hits;
+  return CBM_OK;
+}
+
+int cbm_trigger_device_status(cbm_trigger_t* h, void* stream, cbm_trigger_stats_t* stats) {
+  if (!h) return CBM_ERR_INVALID_ARG;
+  if (!stats) return fail(h, CBM_ERR_INVALID_ARG, "stats must not be NULL");
+  CBM_CUDA(h, cudaSetDevice(h->cfg.device));
+  CBM_CUDA(h, cudaMemcpyAsync(h->h_dev_ctrl, h->dev_scr.d_ctrl, sizeof(Ctrl), cudaMemcpyDeviceToHost, (cudaStream_t)stream));
+  CBM_CUDA(h, cudaStreamSynchronize((cudaStream_t)stream));
+  fill_stats(*stats, *h->h_dev_ctrl, h->dev_n_events, h->dev_n_hits, h->dev_n_events ? 4 : 0);
+  if (h->cfg.flags & CBM_FLAG_PROFILE) fill_prof(*stats, h->dev_prof, false);
+  if (stats->n_invalid)
+    return fail(h, CBM_ERR_RANGE, "%u event(s) rejected on the device; first: event %u", stats->n_invalid, stats->first_invalid);
+  return CBM_OK;
+}
+
+}  // extern "C"

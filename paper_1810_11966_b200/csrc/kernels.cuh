@@ -1,0 +1,513 @@
+// kernels.cuh -- the sm_100a kernels of the CBM-MUCH first-level J/psi selection.
+//
+// Steps a3..a8 of DESIGN.md:
+//   tile_kernel   a3 classify every event (reads off[] once), queue the non-tiny ones by class;
+//                 a4 stage the tiny events of a 32-event tile into shared memory with 1-D TMA bulk copies;
+//                 a5 thread-per-(event,station) triplet search on the staged hits; a8 result write.
+//   team_kernel   persistent, one team (1, 4 or 16 warps) per queued event:
+//                 a4/a5 2-D slope-binned triplet search anchored on the middle layer, a6 ballot/popc
+//                 compaction of compatible (h0,h1) pairs, a7 cross-station chain count, a8 result write.
+//
+// The window test is always the exact int64 inequality (PAPER.md:75-76 with the north_star's window):
+//   |x_h*z_B - x_g*z_A| <= T_AB,  evaluated as  (uint64)(x_h*z_B + T_AB - x_g*z_A) <= 2*T_AB.
+// Slope keys / bins only decide WHERE to look; the bins searched are a proven superset (params.h).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "params.h"
+
+namespace cbm {
+
+// ---------------------------------------------------------------------------------------------- PTX helpers
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void fence_mbar_init() {
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity) {
+  uint32_t ok;
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+      "selp.u32 %0, 1, 0, p;\n\t}"
+      : "=r"(ok)
+      : "r"(smem_u32(bar)), "r"(parity)
+      : "memory");
+  return ok != 0;
+}
+// 1-D TMA bulk copy global -> shared, completion counted in bytes on an mbarrier (SASS: UBLKCP).
+// dst, src 16-byte aligned, bytes a multiple of 16.
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                   smem_u32(dst)),
+               "l"(src), "r"(bytes), "r"(smem_u32(bar))
+               : "memory");
+}
+
+// ---------------------------------------------------------------------------------------------- window test
+// P = a*z_other + T (hoisted per anchor hit);  pass  <=>  |a*z_other - b*z_a| <= T
+__device__ __forceinline__ bool win(int64_t P, int32_t b, int32_t za, uint64_t T2) {
+  return (uint64_t)(P - (int64_t)b * (int64_t)za) <= T2;
+}
+__device__ __forceinline__ uint32_t sat32(unsigned long long v) { return v > (unsigned long long)kSat ? kSat : (uint32_t)v; }
+
+__device__ __forceinline__ uint32_t lanemask_lt() {
+  uint32_t m;
+  asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m));
+  return m;
+}
+
+// ================================================================================================ tile kernel
+// One CTA = kTileEvents (32) consecutive events, blockDim.x = 32*S threads: thread t <-> (event t/S, station t%S).
+struct TileSmem {
+  alignas(16) int32_t sx[kTileHitCap];
+  alignas(16) int32_t sy[kTileHitCap];
+  uint32_t off[kTileEvents * kMaxLayers + 1];
+  uint32_t ev_max[kTileEvents];
+  uint32_t ev_dst[kTileEvents];
+  uint32_t st_cnt[kTileEvents * kMaxStations];
+  alignas(8) uint64_t bar;
+};
+
+__global__ void __launch_bounds__(kTileEvents* kMaxStations)
+    tile_kernel(const __grid_constant__ Params p, const int32_t* __restrict__ x, const int32_t* __restrict__ y,
+                const uint32_t* __restrict__ off, uint32_t n_events, uint32_t n_hits, uint32_t* __restrict__ n_triplets,
+                uint32_t* __restrict__ n_candidates, uint8_t* __restrict__ accept, Ctrl* __restrict__ ctrl,
+                uint32_t* __restrict__ list_M, uint32_t* __restrict__ list_H, uint32_t* __restrict__ list_G) {
+  __shared__ TileSmem sm;
+  const uint32_t tid = threadIdx.x, nthr = blockDim.x;
+  const uint32_t S = p.S, L = p.L;
+  const uint32_t e0 = blockIdx.x * kTileEvents;
+  const uint32_t ne = min((uint32_t)kTileEvents, n_events - e0);
+
+  // ---- a3: offsets of the tile, read once, coalesced
+  {
+    const uint32_t n_off = ne * L + 1;
+    const uint32_t* src = off + (size_t)e0 * L;
+    for (uint32_t i = tid; i < n_off; i += nthr) sm.off[i] = __ldg(src + i);
+  }
+  if (tid < kTileEvents) sm.ev_max[tid] = 0;
+  if (tid == 0) {
+    mbar_init(&sm.bar, 1);
+    fence_mbar_init();
+  }
+  __syncthreads();
+
+  const uint32_t el = tid / S, s = tid - el * S;
+  const bool active = el < ne;
+  uint32_t o0 = 0, o1 = 0, o2 = 0, o3 = 0;
+  if (active) {
+    const uint32_t* o = &sm.off[el * L + 3 * s];
+    o0 = o[0]; o1 = o[1]; o2 = o[2]; o3 = o[3];
+    const bool valid = (o0 <= o1) & (o1 <= o2) & (o2 <= o3) & (o3 <= n_hits);
+    uint32_t mx = max(max(o1 - o0, o2 - o1), o3 - o2);
+    if (!valid || mx > p.max_hits_per_layer) mx = 0xFFFFFFFFu;
+    atomicMax(&sm.ev_max[el], mx);
+  }
+  __syncthreads();
+
+  // ---- planning warp: lane <-> event.  Classes, queues, shared-memory placement, TMA issue.
+  if (tid < 32) {
+    const uint32_t lane = tid;
+    const bool in = lane < ne;
+    const uint32_t mx = in ? sm.ev_max[lane] : 0u;
+    const uint32_t ob = in ? sm.off[lane * L] : 0u, oe = in ? sm.off[(lane + 1) * L] : 0u;
+    const bool invalid = in && mx == 0xFFFFFFFFu;
+    const uint32_t tot = oe - ob;
+    const bool tiny = in && !invalid && p.tiny_max_total != 0 && mx <= p.tiny_max_layer && tot <= p.tiny_max_total;
+    const uint32_t tmask = __ballot_sync(0xFFFFFFFFu, tiny);
+    // my run = maximal block of consecutive tiny events around me; runs are contiguous in x[] / y[]
+    const uint32_t nz_below = (~tmask) & ((1u << lane) - 1u);
+    const uint32_t rs = nz_below ? (32u - __clz(nz_below)) : 0u;  // first lane of my run
+    const uint32_t nz_above = (~tmask) >> lane;                   // bit k: lane+k is not tiny
+    const uint32_t re = nz_above ? (lane + __ffs(nz_above) - 2u) & 31u : 31u;  // last lane of my run
+    const bool start = tiny && rs == lane;
+    const uint32_t run_src = __shfl_sync(0xFFFFFFFFu, ob, rs) & ~3u;  // 16-byte aligned source
+    const uint32_t run_oe = __shfl_sync(0xFFFFFFFFu, oe, re);
+    const uint32_t run_len = start ? (((run_oe + 3u) & ~3u) - run_src) : 0u;  // multiple of 4 hits
+    uint32_t incl = run_len;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+      const uint32_t v = __shfl_up_sync(0xFFFFFFFFu, incl, d);
+      if (lane >= (uint32_t)d) incl += v;
+    }
+    const uint32_t excl = incl - run_len;
+    const uint32_t total = __shfl_sync(0xFFFFFFFFu, incl, 31);  // <= kTileHitCap by construction (params.h)
+    const uint32_t run_dst = __shfl_sync(0xFFFFFFFFu, excl, rs);
+    sm.ev_dst[lane] = tiny ? run_dst + (ob - run_src) : kNotTiny;
+    if (lane == 0) mbar_arrive_expect_tx(&sm.bar, total * 8u);
+    __syncwarp();
+    if (start && run_len) {  // a4: one bulk copy per run and coordinate
+      bulk_g2s(&sm.sx[excl], x + run_src, run_len * 4u, &sm.bar);
+      bulk_g2s(&sm.sy[excl], y + run_src, run_len * 4u, &sm.bar);
+    }
+    // queue the rest by class (order inside a list is irrelevant: results are indexed by event)
+    int cls = -1;
+    if (in && !invalid && !tiny) cls = mx <= p.cls_max[kClsM] ? kClsM : (mx <= p.cls_max[kClsH] ? kClsH : kClsG);
+    uint32_t* const lists[kNumTeamClasses] = {list_M, list_H, list_G};
+#pragma unroll
+    for (int c = 0; c < kNumTeamClasses; ++c) {
+      const uint32_t m = __ballot_sync(0xFFFFFFFFu, cls == c);
+      if (m) {
+        const int leader = __ffs(m) - 1;
+        uint32_t base = 0;
+        if ((int)lane == leader) base = atomicAdd(&ctrl->count[c], __popc(m));
+        base = __shfl_sync(0xFFFFFFFFu, base, leader);
+        if (cls == c) lists[c][base + __popc(m & lanemask_lt())] = e0 + lane;
+      }
+    }
+    if (invalid) {  // rejected on the device: outputs 0, reported by fetch_results / device_status
+      const uint32_t e = e0 + lane;
+      for (uint32_t k = 0; k < S; ++k) n_triplets[(size_t)e * S + k] = 0;
+      n_candidates[e] = 0;
+      accept[e] = 0;
+      atomicAdd(&ctrl->n_invalid, 1u);
+      atomicMax(&ctrl->first_invalid_inv, ~e);
+    }
+  }
+  __syncthreads();
+  while (!mbar_try_wait(&sm.bar, 0)) {
+  }
+
+  // ---- a5: brute-force triplet search of one station of one tiny event per thread (5 x 5 pairs typical)
+  const uint32_t dst = active ? sm.ev_dst[el] : kNotTiny;
+  const bool mine = dst != kNotTiny;
+  uint32_t cnt = 0;
+  if (mine) {
+    const uint32_t shift = dst - sm.off[el * L];  // shared index = global index + shift (mod 2^32)
+    const int32_t z0 = p.z[3 * s], z1 = p.z[3 * s + 1], z2 = p.z[3 * s + 2];
+    const int64_t T01 = p.thr_in[s][0], T02 = p.thr_in[s][1], T12 = p.thr_in[s][2];
+    const uint32_t b0 = o0 + shift, b1 = o1 + shift, b2 = o2 + shift, b3 = o3 + shift;
+    if (b2 != b3) {
+      for (uint32_t i0 = b0; i0 < b1; ++i0) {
+        const int32_t x0 = sm.sx[i0], y0 = sm.sy[i0];
+        const int64_t Px = (int64_t)x0 * z1 + T01, Py = (int64_t)y0 * z1 + T01;
+        for (uint32_t i1 = b1; i1 < b2; ++i1) {
+          const int32_t x1 = sm.sx[i1];
+          if (!win(Px, x1, z0, 2 * (uint64_t)T01)) continue;
+          const int32_t y1 = sm.sy[i1];
+          if (!win(Py, y1, z0, 2 * (uint64_t)T01)) continue;
+          const int64_t Qx0 = (int64_t)x0 * z2 + T02, Qy0 = (int64_t)y0 * z2 + T02;
+          const int64_t Qx1 = (int64_t)x1 * z2 + T12, Qy1 = (int64_t)y1 * z2 + T12;
+          for (uint32_t i2 = b2; i2 < b3; ++i2) {
+            const int32_t x2 = sm.sx[i2], y2 = sm.sy[i2];
+            const bool ok = win(Qx0, x2, z0, 2 * (uint64_t)T02) & win(Qy0, y2, z0, 2 * (uint64_t)T02) &
+                            win(Qx1, x2, z1, 2 * (uint64_t)T12) & win(Qy1, y2, z1, 2 * (uint64_t)T12);
+            cnt += ok ? 1u : 0u;
+          }
+        }
+      }
+    }
+    sm.st_cnt[tid] = cnt;
+    n_triplets[(size_t)e0 * S + tid] = cnt;  // a8: consecutive threads, consecutive addresses
+  }
+  __syncthreads();
+  // ---- a7/a8: a chain needs a triplet in every station.  If some station has none: 0 candidates, done.
+  // Otherwise (rare: essentially only planted tracks) the event is re-queued to class M, whose kernel
+  // recomputes it with the full chain count and overwrites these outputs.
+  if (mine && s == 0) {
+    const uint32_t e = e0 + el;
+    bool all = true;
+    for (uint32_t k = 0; k < S; ++k) all &= sm.st_cnt[el * S + k] != 0;
+    if (!all) {
+      n_candidates[e] = 0;
+      accept[e] = p.min_candidates == 0 ? 1 : 0;
+    } else if (S == 1) {
+      n_candidates[e] = cnt;
+      accept[e] = cnt >= p.min_candidates ? 1 : 0;
+    } else {
+      const uint32_t pos = atomicAdd(&ctrl->count[kClsM], 1u);
+      list_M[pos] = e;
+      atomicAdd(&ctrl->n_escalated, 1u);
+    }
+  }
+}
+
+// ================================================================================================ team kernel
+// One team = one CTA of W warps works on one event at a time (persistent: events are fetched from the class
+// list with an atomic cursor).  CAP = fullest layer the class admits, NC >= nb*nb cells per binned layer.
+template <int W>
+__device__ __forceinline__ void team_sync() {
+  if (W == 1) __syncwarp(); else __syncthreads();
+}
+
+template <int W, int CAP, int NC>
+struct TeamSmem {
+  int32_t sx0[CAP], sy0[CAP];      // layer 0 of the station, bin-sorted
+  int32_t sx2[CAP], sy2[CAP];      // layer 2, bin-sorted
+  uint32_t m[CAP];                 // m[i1] = number of triplets with middle hit i1   (R8: linking sees only h1)
+  int32_t ux[2][CAP], uy[2][CAP];  // distinct middle hits with m > 0 of the previous / current station
+  uint32_t uc[2][CAP];             // their saturated chain counts c_s[u]
+  uint32_t cell0[NC + 1], cell2[NC + 1];  // cell c of the layer = [cell[c], cell[c+1])
+  uint32_t queue[W][64];           // per-warp queue of compatible (h0,h1) pairs: (i0_sorted << 16) | i1
+  uint32_t off[kMaxLayers + 1];
+  uint32_t wsum[32];
+  unsigned long long acc;          // block-wide u64 accumulator (triplet total / candidate total)
+  uint32_t ucount;
+  uint32_t ev;
+};
+
+// in-place exclusive scan of a[1..n] (a[0] stays 0) by the whole team
+template <int W>
+__device__ __forceinline__ void team_exclusive_scan(uint32_t* a, uint32_t n, uint32_t* wsum) {
+  constexpr uint32_t T = 32 * W;
+  const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const uint32_t chunk = (n + T - 1) / T;
+  const uint32_t lo = min(tid * chunk, n), hi = min(lo + chunk, n);
+  uint32_t sum = 0;
+  for (uint32_t i = lo; i < hi; ++i) sum += a[1 + i];
+  uint32_t incl = sum;
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) {
+    const uint32_t v = __shfl_up_sync(0xFFFFFFFFu, incl, d);
+    if (lane >= (uint32_t)d) incl += v;
+  }
+  uint32_t base = incl - sum;
+  if (W > 1) {
+    if (lane == 31) wsum[warp] = incl;
+    __syncthreads();
+    uint32_t wbase = 0;
+    for (uint32_t w = 0; w < warp; ++w) wbase += wsum[w];
+    base += wbase;
+  }
+  for (uint32_t i = lo; i < hi; ++i) {
+    const uint32_t c = a[1 + i];
+    a[1 + i] = base;
+    base += c;
+  }
+}
+
+__device__ __forceinline__ int bin_of(int key, int kmin, int sh, int nbm1) {
+  return min(max((key - kmin) >> sh, 0), nbm1);
+}
+
+// Phase 2 (a5): for one compatible (h0,h1) pair, count the h2 of layer 2 compatible with both.
+// Looks only at the 2-D bins around h1's slope (superset of its window), tests exactly.
+template <class SM>
+__device__ __forceinline__ uint32_t count_h2(const SM& sm, int32_t x0, int32_t y0, int32_t x1, int32_t y1, int32_t z0,
+                                             int32_t z1, int32_t z2, int64_t T02, int64_t T12, int32_t M1, int kmin,
+                                             int R, int sh, int nb) {
+  const int kx = __mulhi(x1, M1), ky = __mulhi(y1, M1);
+  const int bxl = bin_of(kx - R, kmin, sh, nb - 1), bxh = bin_of(kx + R, kmin, sh, nb - 1);
+  const int byl = bin_of(ky - R, kmin, sh, nb - 1), byh = bin_of(ky + R, kmin, sh, nb - 1);
+  const int64_t Qx0 = (int64_t)x0 * z2 + T02, Qy0 = (int64_t)y0 * z2 + T02;
+  const int64_t Qx1 = (int64_t)x1 * z2 + T12, Qy1 = (int64_t)y1 * z2 + T12;
+  uint32_t c = 0;
+  for (int bx = bxl; bx <= bxh; ++bx) {
+    const uint32_t ja = sm.cell2[bx * nb + byl], jb = sm.cell2[bx * nb + byh + 1];
+    for (uint32_t j = ja; j < jb; ++j) {
+      const int32_t x2 = sm.sx2[j], y2 = sm.sy2[j];
+      const bool ok = win(Qx1, x2, z1, 2 * (uint64_t)T12) & win(Qy1, y2, z1, 2 * (uint64_t)T12) &
+                      win(Qx0, x2, z0, 2 * (uint64_t)T02) & win(Qy0, y2, z0, 2 * (uint64_t)T02);
+      c += ok ? 1u : 0u;
+    }
+  }
+  return c;
+}
+
+template <int W, int CAP, int NC, int CLS>
+__global__ void __launch_bounds__(32 * W)
+    team_kernel(const __grid_constant__ Params p, const int32_t* __restrict__ x, const int32_t* __restrict__ y,
+                const uint32_t* __restrict__ off, uint32_t* __restrict__ n_triplets, uint32_t* __restrict__ n_candidates,
+                uint8_t* __restrict__ accept, Ctrl* __restrict__ ctrl, const uint32_t* __restrict__ list) {
+  using SM = TeamSmem<W, CAP, NC>;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  SM& sm = *reinterpret_cast<SM*>(smem_raw);
+  constexpr uint32_t T = 32 * W;
+  const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const uint32_t S = p.S, L = p.L;
+  const uint32_t n_list = ctrl->count[CLS];
+  const int kmin = p.key_min, R = p.key_R, sh = p.cls_shift[CLS], nb = (int)p.cls_nb[CLS];
+  const uint32_t ncell = (uint32_t)(nb * nb);
+
+  for (;;) {
+    if (tid == 0) sm.ev = atomicAdd(&ctrl->work[CLS], 1u);
+    team_sync<W>();
+    const uint32_t li = sm.ev;
+    if (li >= n_list) break;
+    const uint32_t e = list[li];
+    for (uint32_t i = tid; i <= L; i += T) sm.off[i] = __ldg(off + (size_t)e * L + i);
+    team_sync<W>();
+
+    uint32_t nprev = 0;
+    bool dead = false;  // some station so far has no triplet => no chain; triplet counts are still needed
+    int cur = 0;
+    for (uint32_t s = 0; s < S; ++s) {
+      const uint32_t b0 = sm.off[3 * s], b1 = sm.off[3 * s + 1], b2 = sm.off[3 * s + 2], b3 = sm.off[3 * s + 3];
+      const uint32_t n0 = b1 - b0, n1 = b2 - b1, n2 = b3 - b2;
+      const int32_t z0 = p.z[3 * s], z1 = p.z[3 * s + 1], z2 = p.z[3 * s + 2];
+      const int32_t M0 = p.key_mul[3 * s], M1 = p.key_mul[3 * s + 1], M2 = p.key_mul[3 * s + 2];
+      const int64_t T01 = p.thr_in[s][0], T02 = p.thr_in[s][1], T12 = p.thr_in[s][2];
+      if (tid == 0) { sm.acc = 0; sm.ucount = 0; }
+      bool any_triplet_possible = (n0 != 0) & (n1 != 0) & (n2 != 0);
+      if (any_triplet_possible) {
+        // ---- a4: bin layers 0 and 2 on a 2-D slope grid (count, scan, scatter)
+        for (uint32_t i = tid; i <= ncell; i += T) { sm.cell0[i] = 0; sm.cell2[i] = 0; }
+        for (uint32_t i = tid; i < n1; i += T) sm.m[i] = 0;
+        team_sync<W>();
+        for (uint32_t i = tid; i < n0 + n2; i += T) {
+          const bool l2 = i >= n0;
+          const uint32_t g = l2 ? b2 + (i - n0) : b0 + i;
+          const int32_t hx = __ldg(x + g), hy = __ldg(y + g);
+          const int32_t M = l2 ? M2 : M0;
+          const int c = bin_of(__mulhi(hx, M), kmin, sh, nb - 1) * nb + bin_of(__mulhi(hy, M), kmin, sh, nb - 1);
+          atomicAdd(l2 ? &sm.cell2[c + 1] : &sm.cell0[c + 1], 1u);
+        }
+        team_sync<W>();
+        team_exclusive_scan<W>(sm.cell0, ncell, sm.wsum);
+        team_sync<W>();
+        team_exclusive_scan<W>(sm.cell2, ncell, sm.wsum);
+        team_sync<W>();
+        for (uint32_t i = tid; i < n0 + n2; i += T) {
+          const bool l2 = i >= n0;
+          const uint32_t g = l2 ? b2 + (i - n0) : b0 + i;
+          const int32_t hx = __ldg(x + g), hy = __ldg(y + g);
+          const int32_t M = l2 ? M2 : M0;
+          const int c = bin_of(__mulhi(hx, M), kmin, sh, nb - 1) * nb + bin_of(__mulhi(hy, M), kmin, sh, nb - 1);
+          if (l2) {
+            const uint32_t pos = atomicAdd(&sm.cell2[c + 1], 1u);
+            sm.sx2[pos] = hx; sm.sy2[pos] = hy;
+          } else {
+            const uint32_t pos = atomicAdd(&sm.cell0[c + 1], 1u);
+            sm.sx0[pos] = hx; sm.sy0[pos] = hy;
+          }
+        }
+        team_sync<W>();
+
+        // ---- a5/a6: anchors = middle-layer hits, one per lane; compatible (h0,h1) pairs are compacted
+        // into the warp's queue with ballot/popc and drained 32 at a time by phase 2.
+        uint32_t qn = 0;
+        uint32_t* const q = sm.queue[warp];
+        for (uint32_t base = warp * 32; base < n1; base += T) {
+          const uint32_t i1 = base + lane;
+          const bool act = i1 < n1;
+          int32_t x1 = 0, y1 = 0;
+          int bx = 0, bxh = -1, byl = 0, byh = 0;
+          uint32_t j = 0, jend = 0;
+          if (act) {
+            x1 = __ldg(x + b1 + i1); y1 = __ldg(y + b1 + i1);
+            const int kx = __mulhi(x1, M1), ky = __mulhi(y1, M1);
+            bx = bin_of(kx - R, kmin, sh, nb - 1) - 1;  // advanced to the first row below
+            bxh = bin_of(kx + R, kmin, sh, nb - 1);
+            byl = bin_of(ky - R, kmin, sh, nb - 1);
+            byh = bin_of(ky + R, kmin, sh, nb - 1);
+          }
+          // |x0*z1 - x1*z0| <= T01  <=>  (uint64)(x0*z1 + (T01 - x1*z0)) <= 2*T01
+          const int64_t Qx = T01 - (int64_t)x1 * z0, Qy = T01 - (int64_t)y1 * z0;
+          for (;;) {
+            if (j >= jend && bx < bxh) {  // next row of bins
+              ++bx;
+              j = sm.cell0[bx * nb + byl];
+              jend = sm.cell0[bx * nb + byh + 1];
+            }
+            const bool more = (j < jend) | (bx < bxh);
+            if (!__any_sync(0xFFFFFFFFu, more)) break;
+            bool pass = false;
+            if (j < jend) {
+              const int32_t hx = sm.sx0[j];
+              if ((uint64_t)((int64_t)hx * z1 + Qx) <= 2 * (uint64_t)T01) {
+                const int32_t hy = sm.sy0[j];
+                pass = (uint64_t)((int64_t)hy * z1 + Qy) <= 2 * (uint64_t)T01;
+              }
+            }
+            const uint32_t pm = __ballot_sync(0xFFFFFFFFu, pass);
+            if (pm) {
+              if (pass) q[qn + __popc(pm & lanemask_lt())] = (j << 16) | i1;
+              qn += __popc(pm);
+              if (qn >= 32) {
+                __syncwarp();
+                qn -= 32;
+                const uint32_t ent = q[qn + lane];
+                const uint32_t j0 = ent >> 16, k1 = ent & 0xFFFFu;
+                const uint32_t c = count_h2(sm, sm.sx0[j0], sm.sy0[j0], __ldg(x + b1 + k1), __ldg(y + b1 + k1), z0, z1,
+                                            z2, T02, T12, M1, kmin, R, sh, nb);
+                if (c) atomicAdd(&sm.m[k1], c);
+                __syncwarp();
+              }
+            }
+            if (j < jend) ++j;
+          }
+        }
+        __syncwarp();
+        if (lane < qn) {
+          const uint32_t ent = q[lane];
+          const uint32_t j0 = ent >> 16, k1 = ent & 0xFFFFu;
+          const uint32_t c = count_h2(sm, sm.sx0[j0], sm.sy0[j0], __ldg(x + b1 + k1), __ldg(y + b1 + k1), z0, z1, z2,
+                                      T02, T12, M1, kmin, R, sh, nb);
+          if (c) atomicAdd(&sm.m[k1], c);
+        }
+      }
+      team_sync<W>();
+
+      // ---- station total, list of distinct middle hits with triplets (R8)
+      if (any_triplet_possible) {
+        unsigned long long part = 0;
+        for (uint32_t i = tid; i < n1; i += T) {
+          const uint32_t mm = sm.m[i];
+          part += mm;
+          if (mm && !dead) {
+            const uint32_t pos = atomicAdd(&sm.ucount, 1u);
+            sm.ux[cur][pos] = __ldg(x + b1 + i);
+            sm.uy[cur][pos] = __ldg(y + b1 + i);
+            sm.uc[cur][pos] = mm;
+          }
+        }
+#pragma unroll
+        for (int d = 16; d >= 1; d >>= 1) part += __shfl_xor_sync(0xFFFFFFFFu, part, d);
+        if (lane == 0 && part) atomicAdd(&sm.acc, part);
+      }
+      team_sync<W>();
+      const uint32_t ncur = dead ? 0u : sm.ucount;
+      if (tid == 0) n_triplets[(size_t)e * S + s] = sat32(sm.acc);
+      // ---- a7: chain counts c_s[u] = m_u * sum over linked t of c_{s-1}[t], saturating (R9)
+      if (s > 0 && !dead && ncur) {
+        const int32_t zA = p.z[3 * (s - 1) + 1], zB = z1;
+        const int64_t TL = p.thr_link[s];
+        for (uint32_t u = tid; u < ncur; u += T) {
+          const int32_t xu = sm.ux[cur][u], yu = sm.uy[cur][u];
+          // |x_t*zB - x_u*zA| <= TL
+          const int64_t Qx = TL - (int64_t)xu * zA, Qy = TL - (int64_t)yu * zA;
+          unsigned long long a = 0;
+          for (uint32_t t = 0; t < nprev; ++t) {
+            const bool ok = ((uint64_t)((int64_t)sm.ux[cur ^ 1][t] * zB + Qx) <= 2 * (uint64_t)TL) &
+                            ((uint64_t)((int64_t)sm.uy[cur ^ 1][t] * zB + Qy) <= 2 * (uint64_t)TL);
+            if (ok) a += sm.uc[cur ^ 1][t];  // < 4096 * 2^32
+          }
+          a = sat32(a);
+          sm.uc[cur][u] = sat32(a * (unsigned long long)sm.uc[cur][u]);  // m_u <= 2^24: no overflow
+        }
+      }
+      if (ncur == 0) dead = true;
+      nprev = ncur;
+      cur ^= 1;
+      team_sync<W>();
+    }
+
+    // ---- candidates = sum over the last station's middle hits; a8: one writer per event
+    if (tid == 0) sm.acc = 0;
+    team_sync<W>();
+    if (!dead) {
+      unsigned long long part = 0;
+      for (uint32_t u = tid; u < nprev; u += T) part += sm.uc[cur ^ 1][u];
+#pragma unroll
+      for (int d = 16; d >= 1; d >>= 1) part += __shfl_xor_sync(0xFFFFFFFFu, part, d);
+      if (lane == 0 && part) atomicAdd(&sm.acc, part);
+    }
+    team_sync<W>();
+    if (tid == 0) {
+      const uint32_t c = sat32(sm.acc);
+      n_candidates[e] = c;
+      accept[e] = c >= p.min_candidates ? 1 : 0;
+    }
+    team_sync<W>();
+  }
+}
+
+}  // namespace cbm

@@ -1,0 +1,57 @@
+// params.h -- plain-old-data shared by the host side (cbm_trigger.cu) and the kernels (kernels.cuh).
+//
+// Everything the kernels need about the geometry and the windows is precomputed once on the host at
+// cbm_trigger_create() and passed to every launch by value (__grid_constant__).
+#pragma once
+#include <stdint.h>
+
+namespace cbm {
+
+constexpr int kMaxStations = 8;
+constexpr int kMaxLayers = 24;
+constexpr uint32_t kSat = 0xFFFFFFFFu;       // outputs are min(2^32-1, exact)  (R9, R12)
+constexpr uint32_t kNotTiny = 0xFFFFFFFFu;
+
+// Event classes of the scheduler: tiny events are finished by the tile kernel,
+// the others are queued for a team kernel with a team size and a shared-memory budget that fits them.
+constexpr int kNumTeamClasses = 3;           // M, H, G
+constexpr int kClsM = 0, kClsH = 1, kClsG = 2;
+
+struct Params {
+  uint32_t S, L;
+  int32_t z[kMaxLayers];               // layer z, 10-um units
+  // window thresholds, R4: |x_h*z_B - x_g*z_A| <= T_AB = floor(a*z_A*z_B / b)  (left side is an integer)
+  int64_t thr_in[kMaxStations][3];     // [s][0] = T01, [1] = T02, [2] = T12
+  int64_t thr_link[kMaxStations];      // [s], s >= 1: middle layers of stations s-1 and s
+  // slope keys used ONLY to choose which bins to look at (never to accept or reject a pair):
+  // key(x, l) = mulhi(x, key_mul[l]) = floor(x * key_mul[l] / 2^32) ~ K * x / z_l, with |key - K*x/z_l| < 1.25
+  int32_t key_mul[kMaxLayers];
+  int32_t key_min;                     // key of slope -slope_range
+  int32_t key_R;                       // two x- (or y-) compatible hits have |key_h - key_g| <= key_R
+  int32_t cls_shift[kNumTeamClasses];  // bin = clamp((key - key_min) >> shift, 0, nb-1); 2*key_R <= 2^shift
+  uint32_t cls_nb[kNumTeamClasses];    // bins per axis (grid is nb x nb per layer)
+  uint32_t cls_max[kNumTeamClasses];   // fullest layer an event of this class may have
+  uint32_t min_candidates;
+  uint32_t max_hits_per_layer;
+  uint32_t tiny_max_layer;             // 0 disables the tiny path
+  uint32_t tiny_max_total;
+};
+
+// Device-resident scheduler state of one run; zero-initialised by cudaMemsetAsync before the tile kernel.
+struct Ctrl {
+  uint32_t count[kNumTeamClasses];     // list lengths (written by the tile kernel)
+  uint32_t work[kNumTeamClasses];      // work-fetch cursors of the persistent team kernels
+  uint32_t n_invalid;
+  uint32_t first_invalid_inv;          // max over invalid events of ~event  (0 = none)
+  uint32_t n_escalated;                // tiny events with a triplet in every station, re-queued to class M
+  uint32_t pad[7];
+};
+static_assert(sizeof(Ctrl) == 64, "Ctrl is copied as one 64-byte record");
+
+// tile kernel geometry
+constexpr int kTileEvents = 32;              // events per CTA of the tile kernel = lanes of the planning warp
+constexpr uint32_t kTinyMaxTotal = 96;       // a tiny event holds at most this many hits ...
+constexpr uint32_t kTileHitCap = kTileEvents * kTinyMaxTotal + 32;  // ... so a tile never overflows this (see tile_kernel)
+constexpr uint32_t kTinyMaxLayerLimit = 32;
+
+}  // namespace cbm

@@ -1,0 +1,87 @@
+"""Shared helpers of the parity tests: a multi-threaded driver of the CPU oracle (events are
+independent) and a one-call wrapper of the CUDA path through the C ABI."""
+import os
+from concurrent.futures import ThreadPoolExecutor
+
+import numpy as np
+
+import oracle
+from paper_1810_11966_b200 import binding as K
+
+
+def oracle_mt(geo, x, y, off, e_begin=0, e_end=None, n_threads=None, chunk=2000):
+    """oracle.run over [e_begin, e_end) on all host cores (ctypes releases the GIL)."""
+    S = geo.n_stations
+    n_events = (off.size - 1) // (3 * S)
+    e_end = n_events if e_end is None else e_end
+    n = e_end - e_begin
+    nt = np.zeros((n, S), dtype=np.uint32)
+    nc = np.zeros(n, dtype=np.uint32)
+    ac = np.zeros(n, dtype=np.uint8)
+    n_threads = n_threads or min(32, os.cpu_count() or 1)
+    ranges = [(a, min(a + chunk, e_end)) for a in range(e_begin, e_end, chunk)]
+
+    def work(r):
+        a, b = r
+        t, c, k = oracle.run(geo, x, y, off, a, b)
+        nt[a - e_begin:b - e_begin] = t
+        nc[a - e_begin:b - e_begin] = c
+        ac[a - e_begin:b - e_begin] = k
+
+    with ThreadPoolExecutor(n_threads) as ex:
+        list(ex.map(work, ranges))
+    return nt, nc, ac
+
+
+def oracle_list_mt(geo, x, y, off, ids, n_threads=None):
+    ids = np.asarray(ids, dtype=np.uint64)
+    S = geo.n_stations
+    n_threads = n_threads or min(32, os.cpu_count() or 1)
+    parts = np.array_split(np.arange(ids.size), max(1, min(ids.size, n_threads * 4)))
+    nt = np.zeros((ids.size, S), dtype=np.uint32)
+    nc = np.zeros(ids.size, dtype=np.uint32)
+    ac = np.zeros(ids.size, dtype=np.uint8)
+
+    def work(p):
+        if p.size == 0:
+            return
+        t, c, k = oracle.run_list(geo, x, y, off, ids[p])
+        nt[p], nc[p], ac[p] = t, c, k
+
+    with ThreadPoolExecutor(n_threads) as ex:
+        list(ex.map(work, parts))
+    return nt, nc, ac
+
+
+def gpu_select(layer_z, x, y, off, win_in=(1, 100), win_link=(2, 100), min_candidates=2, max_hits_per_layer=4096,
+               flags=0, tiny_max_layer_hits=0, slope_range_milli=0, check=True):
+    """One batch through cbm_trigger_create / upload_events / run / fetch_results."""
+    L = len(layer_z)
+    n_events = (off.size - 1) // L
+    n_hits = int(off[-1])
+    trig = K.Trigger(layer_z, max(n_events, 1), max(n_hits, 1), win_in=win_in, win_link=win_link,
+                     min_candidates=min_candidates, max_hits_per_layer=max_hits_per_layer, n_slots=1, flags=flags,
+                     tiny_max_layer_hits=tiny_max_layer_hits, slope_range_milli=slope_range_milli)
+    try:
+        x = np.ascontiguousarray(x, dtype=np.int32)
+        y = np.ascontiguousarray(y, dtype=np.int32)
+        off = np.ascontiguousarray(off, dtype=np.uint32)
+        trig.upload_events(0, x, y, off, n_events, n_hits)
+        trig.run(0)
+        if check:
+            out = trig.fetch_results(0, n_events)
+            return out + (trig.stats(0).as_dict(),)
+        out, rc = trig.fetch_results(0, n_events, check=False)
+        return out + (trig.stats(0).as_dict(), rc, K.cbm_trigger_last_error(trig.handle))
+    finally:
+        trig.close()
+
+
+def assert_same(got, want, what=""):
+    for name, g, w in zip(("n_triplets", "n_candidates", "accept"), got[:3], want[:3]):
+        g = np.asarray(g)
+        w = np.asarray(w).reshape(g.shape)
+        if not np.array_equal(g, w):
+            bad = np.argwhere(g != w)
+            first = tuple(bad[0])
+            raise AssertionError(f"{what}: {name} differs at {len(bad)} places; first {first}: gpu {g[first]} oracle {w[first]}")
