@@ -46,6 +46,7 @@ extern "C" {
 #define CBM_TRIGGER_MAX_HITS_PER_LAYER 4096
 #define CBM_TRIGGER_MAX_SLOTS 4
 #define CBM_TRIGGER_N_KERNELS 4 /* tile, team_M, team_H, team_G (see cbm_trigger_stats_t) */
+#define CBM_TRIGGER_PROFILE_RING 32 /* run_device calls whose per-kernel times are kept (CBM_FLAG_PROFILE) */
 
 enum {
   CBM_OK = 0,
@@ -143,6 +144,12 @@ int cbm_trigger_run_device(cbm_trigger_t* h, uint32_t n_events, uint64_t n_hits,
 /* Synchronises `stream` and fills *stats (HOST) for the last cbm_trigger_run_device call.  Returns
  * CBM_ERR_RANGE if that run rejected events, CBM_OK otherwise. */
 int cbm_trigger_device_status(cbm_trigger_t* h, void* stream, cbm_trigger_stats_t* stats);
+
+/* CBM_FLAG_PROFILE only: synchronises `stream`, then writes the device time in ms of every kernel of the last
+ * min(n_last, CBM_TRIGGER_PROFILE_RING, calls so far) cbm_trigger_run_device calls, oldest first, to the HOST
+ * array kernel_ms[call*CBM_TRIGGER_N_KERNELS + kernel] (CUDA events recorded on the launching stream).
+ * Returns the number of calls written (>= 0) or a negative error code. */
+int cbm_trigger_device_kernel_times(cbm_trigger_t* h, void* stream, uint32_t n_last, float* kernel_ms);
 
 /* Statistics of the last completed run of `slot` (call after fetch_results).  stats: HOST. */
 int cbm_trigger_get_stats(cbm_trigger_t* h, uint32_t slot, cbm_trigger_stats_t* stats);

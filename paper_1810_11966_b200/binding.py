@@ -22,8 +22,9 @@ CBM_FLAG_PROFILE, CBM_FLAG_NO_TINY_PATH = 1, 2
 EXPORTS = (
     "cbm_trigger_create", "cbm_trigger_destroy", "cbm_trigger_host_buffers", "cbm_trigger_upload_events",
     "cbm_trigger_run", "cbm_trigger_fetch_results", "cbm_trigger_run_device", "cbm_trigger_device_status",
-    "cbm_trigger_get_stats", "cbm_trigger_last_error", "cbm_trigger_version",
+    "cbm_trigger_get_stats", "cbm_trigger_last_error", "cbm_trigger_version", "cbm_trigger_device_kernel_times",
 )
+PROFILE_RING = 32
 
 
 class Config(ctypes.Structure):
@@ -99,6 +100,8 @@ def load_library():
         lib.cbm_trigger_run_device.argtypes = [vp, u32, u64, vp, vp, vp, vp, vp, vp, vp]
         lib.cbm_trigger_device_status.restype = i32
         lib.cbm_trigger_device_status.argtypes = [vp, vp, ctypes.POINTER(Stats)]
+        lib.cbm_trigger_device_kernel_times.restype = i32
+        lib.cbm_trigger_device_kernel_times.argtypes = [vp, vp, u32, vp]
         lib.cbm_trigger_get_stats.restype = i32
         lib.cbm_trigger_get_stats.argtypes = [vp, u32, ctypes.POINTER(Stats)]
         lib.cbm_trigger_last_error.restype = ctypes.c_char_p
@@ -208,6 +211,15 @@ def cbm_trigger_device_status(handle, stream=0):
     return rc, st
 
 
+def cbm_trigger_device_kernel_times(handle, stream=0, n_last=PROFILE_RING):
+    """(n, N_KERNELS) float32 array: device ms of every kernel of the last n run_device calls, oldest first."""
+    buf = np.zeros((PROFILE_RING, N_KERNELS), dtype=np.float32)
+    n = load_library().cbm_trigger_device_kernel_times(handle, stream, min(n_last, PROFILE_RING), buf.ctypes.data)
+    if n < 0:
+        _check(n, handle)
+    return buf[:n]
+
+
 # ------------------------------------------------------------------ convenience wrapper
 class Trigger:
     """Owns one handle.  Host-path: upload/run/fetch on slots.  Device path: run_device on torch tensors."""
@@ -271,6 +283,11 @@ class Trigger:
         st = torch.cuda.current_stream().cuda_stream if stream is None else stream
         cbm_trigger_run_device(self.handle, n_events, n_hits, d_x.data_ptr(), d_y.data_ptr(), d_off.data_ptr(),
                                d_nt.data_ptr(), d_nc.data_ptr(), d_ac.data_ptr(), st)
+
+    def device_kernel_times(self, stream=None, n_last=PROFILE_RING):
+        import torch
+        st = torch.cuda.current_stream().cuda_stream if stream is None else stream
+        return cbm_trigger_device_kernel_times(self.handle, st, n_last)
 
     def device_status(self, stream=None):
         import torch

@@ -71,7 +71,8 @@ struct cbm_trigger {
   Slot slot[CBM_TRIGGER_MAX_SLOTS];
   Scratch dev_scr;          // scratch of cbm_trigger_run_device
   Ctrl* h_dev_ctrl = nullptr;
-  ProfEvents dev_prof;
+  ProfEvents dev_prof[CBM_TRIGGER_PROFILE_RING];  // CBM_FLAG_PROFILE: event sets of the last run_device calls
+  uint32_t dev_prof_head = 0;                       // number of run_device calls so far
   uint32_t dev_n_events = 0;
   uint64_t dev_n_hits = 0;
   cudaStream_t st_h2d = nullptr, st_run = nullptr, st_d2h = nullptr;
@@ -370,7 +371,8 @@ int cbm_trigger_create(const cbm_trigger_config_t* cfg, cbm_trigger_t** out) {
   CREATE_CUDA(cudaStreamCreateWithFlags(&h->st_d2h, cudaStreamNonBlocking));
   CREATE_TRY(alloc_scratch(h, h->dev_scr));
   CREATE_CUDA(cudaHostAlloc(&h->h_dev_ctrl, sizeof(Ctrl), cudaHostAllocDefault));
-  if (cfg->flags & CBM_FLAG_PROFILE) CREATE_TRY(make_prof(h, h->dev_prof));
+  if (cfg->flags & CBM_FLAG_PROFILE)
+    for (auto& pe : h->dev_prof) CREATE_TRY(make_prof(h, pe));
   for (uint32_t i = 0; i < cfg->n_slots; ++i) CREATE_TRY(alloc_slot(h, h->slot[i]));
 #undef CREATE_TRY
 #undef CREATE_CUDA
@@ -388,7 +390,7 @@ void cbm_trigger_destroy(cbm_trigger_t* h) {
   }
   for (auto& s : h->slot) free_slot(s);
   free_scratch(h->dev_scr);
-  free_prof(h->dev_prof);
+  for (auto& pe : h->dev_prof) free_prof(pe);
   if (h->h_dev_ctrl) cudaFreeHost(h->h_dev_ctrl);
   if (h->st_h2d) cudaStreamDestroy(h->st_h2d);
   if (h->st_run) cudaStreamDestroy(h->st_run);
@@ -518,9 +520,11 @@ int cbm_trigger_run_device(cbm_trigger_t* h, uint32_t n_events, uint64_t n_hits,
     return fail(h, CBM_ERR_INVALID_ARG, "device pointers must not be NULL");
   if (((uintptr_t)d_x | (uintptr_t)d_y) & 15) return fail(h, CBM_ERR_INVALID_ARG, "d_x and d_y must be 16-byte aligned");
   CBM_CUDA(h, cudaSetDevice(h->cfg.device));
+  ProfEvents* pe = (h->cfg.flags & CBM_FLAG_PROFILE) ? &h->dev_prof[h->dev_prof_head % CBM_TRIGGER_PROFILE_RING] : nullptr;
   const int nl = launch_selection(h, h->dev_scr, d_x, d_y, d_off, n_events, n_hits, d_n_triplets, d_n_candidates,
-                                  d_accept, (cudaStream_t)stream, (h->cfg.flags & CBM_FLAG_PROFILE) ? &h->dev_prof : nullptr);
+                                  d_accept, (cudaStream_t)stream, pe);
   if (nl < 0) return nl;
+  ++h->dev_prof_head;
   h->dev_n_events = n_events;
   h->dev_n_hits = n_hits;
   return CBM_OK;
@@ -533,10 +537,31 @@ int cbm_trigger_device_status(cbm_trigger_t* h, void* stream, cbm_trigger_stats_
   CBM_CUDA(h, cudaMemcpyAsync(h->h_dev_ctrl, h->dev_scr.d_ctrl, sizeof(Ctrl), cudaMemcpyDeviceToHost, (cudaStream_t)stream));
   CBM_CUDA(h, cudaStreamSynchronize((cudaStream_t)stream));
   fill_stats(*stats, *h->h_dev_ctrl, h->dev_n_events, h->dev_n_hits, h->dev_n_events ? 4 : 0);
-  if (h->cfg.flags & CBM_FLAG_PROFILE) fill_prof(*stats, h->dev_prof, false);
+  if ((h->cfg.flags & CBM_FLAG_PROFILE) && h->dev_prof_head)
+    fill_prof(*stats, h->dev_prof[(h->dev_prof_head - 1) % CBM_TRIGGER_PROFILE_RING], false);
   if (stats->n_invalid)
     return fail(h, CBM_ERR_RANGE, "%u event(s) rejected on the device; first: event %u", stats->n_invalid, stats->first_invalid);
   return CBM_OK;
+}
+
+int cbm_trigger_device_kernel_times(cbm_trigger_t* h, void* stream, uint32_t n_last, float* kernel_ms) {
+  if (!h) return CBM_ERR_INVALID_ARG;
+  if (!kernel_ms) return fail(h, CBM_ERR_INVALID_ARG, "kernel_ms must not be NULL");
+  if (!(h->cfg.flags & CBM_FLAG_PROFILE)) return fail(h, CBM_ERR_STATE, "the handle was created without CBM_FLAG_PROFILE");
+  CBM_CUDA(h, cudaSetDevice(h->cfg.device));
+  CBM_CUDA(h, cudaStreamSynchronize((cudaStream_t)stream));
+  uint32_t n = n_last;
+  if (n > CBM_TRIGGER_PROFILE_RING) n = CBM_TRIGGER_PROFILE_RING;
+  if (n > h->dev_prof_head) n = h->dev_prof_head;
+  for (uint32_t i = 0; i < n; ++i) {
+    ProfEvents& pe = h->dev_prof[(h->dev_prof_head - n + i) % CBM_TRIGGER_PROFILE_RING];
+    for (int k = 0; k < CBM_TRIGGER_N_KERNELS; ++k) {
+      float ms = 0;
+      if (pe.valid) CBM_CUDA(h, cudaEventElapsedTime(&ms, pe.k[k], pe.k[k + 1]));
+      kernel_ms[i * CBM_TRIGGER_N_KERNELS + k] = ms;
+    }
+  }
+  return (int)n;
 }
 
 }  // extern "C"

@@ -185,22 +185,33 @@ __global__ void __launch_bounds__(kTileEvents* kMaxStations)
     const int32_t z0 = p.z[3 * s], z1 = p.z[3 * s + 1], z2 = p.z[3 * s + 2];
     const int64_t T01 = p.thr_in[s][0], T02 = p.thr_in[s][1], T12 = p.thr_in[s][2];
     const uint32_t b0 = o0 + shift, b1 = o1 + shift, b2 = o2 + shift, b3 = o3 + shift;
-    if (b2 != b3) {
-      for (uint32_t i0 = b0; i0 < b1; ++i0) {
-        const int32_t x0 = sm.sx[i0], y0 = sm.sy[i0];
-        const int64_t Px = (int64_t)x0 * z1 + T01, Py = (int64_t)y0 * z1 + T01;
-        for (uint32_t i1 = b1; i1 < b2; ++i1) {
-          const int32_t x1 = sm.sx[i1];
-          if (!win(Px, x1, z0, 2 * (uint64_t)T01)) continue;
+    // one flat loop over the n0*n1 (h0,h1) pairs: lanes of a warp run max(n0*n1) iterations instead of
+    // max(n0)*max(n1) (nested loops diverge twice)
+    const uint32_t n_pairs = (b2 != b3) ? (b1 - b0) * (b2 - b1) : 0u;
+    if (n_pairs) {
+      uint32_t i0 = b0, i1 = b1;
+      int32_t x0 = sm.sx[i0], y0 = sm.sy[i0];
+      int64_t Px = (int64_t)x0 * z1 + T01, Py = (int64_t)y0 * z1 + T01;
+      for (uint32_t pr = 0; pr < n_pairs; ++pr) {
+        const int32_t x1 = sm.sx[i1];
+        if (win(Px, x1, z0, 2 * (uint64_t)T01)) {
           const int32_t y1 = sm.sy[i1];
-          if (!win(Py, y1, z0, 2 * (uint64_t)T01)) continue;
-          const int64_t Qx0 = (int64_t)x0 * z2 + T02, Qy0 = (int64_t)y0 * z2 + T02;
-          const int64_t Qx1 = (int64_t)x1 * z2 + T12, Qy1 = (int64_t)y1 * z2 + T12;
-          for (uint32_t i2 = b2; i2 < b3; ++i2) {
-            const int32_t x2 = sm.sx[i2], y2 = sm.sy[i2];
-            const bool ok = win(Qx0, x2, z0, 2 * (uint64_t)T02) & win(Qy0, y2, z0, 2 * (uint64_t)T02) &
-                            win(Qx1, x2, z1, 2 * (uint64_t)T12) & win(Qy1, y2, z1, 2 * (uint64_t)T12);
-            cnt += ok ? 1u : 0u;
+          if (win(Py, y1, z0, 2 * (uint64_t)T01)) {
+            const int64_t Qx0 = (int64_t)x0 * z2 + T02, Qy0 = (int64_t)y0 * z2 + T02;
+            const int64_t Qx1 = (int64_t)x1 * z2 + T12, Qy1 = (int64_t)y1 * z2 + T12;
+            for (uint32_t i2 = b2; i2 < b3; ++i2) {
+              const int32_t x2 = sm.sx[i2], y2 = sm.sy[i2];
+              const bool ok = win(Qx0, x2, z0, 2 * (uint64_t)T02) & win(Qy0, y2, z0, 2 * (uint64_t)T02) &
+                              win(Qx1, x2, z1, 2 * (uint64_t)T12) & win(Qy1, y2, z1, 2 * (uint64_t)T12);
+              cnt += ok ? 1u : 0u;
+            }
+          }
+        }
+        if (++i1 == b2) {
+          i1 = b1;
+          if (++i0 < b1) {
+            x0 = sm.sx[i0]; y0 = sm.sy[i0];
+            Px = (int64_t)x0 * z1 + T01; Py = (int64_t)y0 * z1 + T01;
           }
         }
       }
