@@ -117,7 +117,7 @@ def algorithmic_bytes(n_events, n_hits, S):
     return 8 * n_hits + 4 * (n_events * L + 1) + n_events * (4 * S + 5)
 
 
-def class_accounting(off, S, tiny_max_layer=24, tiny_max_total=96, caps=(128, 512, 4096)):
+def class_accounting(off, S, tiny_max_layer, tiny_max_total, caps):
     """Events, hits and algorithmic bytes per scheduler class (tile, team_M, team_H, team_G), from the offsets.
     Restates the scheduler's rule for the roofline bookkeeping only; the counts are
     checked against the library's own statistics."""
@@ -157,7 +157,7 @@ def oracle_events_per_second(cfg, batch, n_sample, n_threads):
 
 def cpu_sample_size(cid):
     # about 10-30 s of CPU work at the oracle's measured single-core rates
-    return {0: 1000, 1: 200_000, 2: 100_000, 3: 250_000, 4: 100_000}[cid]
+    return {0: 1000, 1: 200_000, 2: 100_000, 3: 500_000, 4: 100_000}[cid]
 
 
 def run_reference(args, cfg, cid):
@@ -288,7 +288,7 @@ def run_ours(args, cfg, cid):
     peak, peak_src = measured_peaks()
 
     # ---- roofline of the dominant kernel: algorithmic bytes of the events it processes / its mean launch time
-    acct = class_accounting(batch.off, S)
+    acct = class_accounting(batch.off, S, K.TINY_MAX_LAYER_DEFAULT, K.TINY_MAX_TOTAL, K.CLASS_CAPS)
     kmean = ktimes.mean(axis=0) if len(ktimes) else np.zeros(4)
     dom = int(np.argmax(kmean))
     # the tile kernel also reads every event's offsets (classification) and writes the tiny events' results

@@ -25,6 +25,9 @@ EXPORTS = (
     "cbm_trigger_get_stats", "cbm_trigger_last_error", "cbm_trigger_version", "cbm_trigger_device_kernel_times",
 )
 PROFILE_RING = 32
+# scheduler classes (csrc/cbm_trigger.cu, csrc/params.h), restated for bookkeeping in bench.py only
+CLASS_CAPS = (128, 448, 4096)
+TINY_MAX_LAYER_DEFAULT, TINY_MAX_TOTAL = 24, 96
 
 
 class Config(ctypes.Structure):

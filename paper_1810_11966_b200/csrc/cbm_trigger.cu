@@ -21,19 +21,25 @@ namespace {
 
 using namespace cbm;
 
-// team classes: warps per team, fullest layer admitted, cells per binned layer
-constexpr int kWM = 1, kCapM = 128, kNcM = 576;
-constexpr int kWH = 4, kCapH = 512, kNcH = 2304;
-constexpr int kWG = 16, kCapG = 4096, kNcG = 2304;
-using SmemM = TeamSmem<kWM, kCapM, kNcM>;
-using SmemH = TeamSmem<kWH, kCapH, kNcH>;
-using SmemG = TeamSmem<kWG, kCapG, kNcG>;
+// team classes: warps per team, fullest layer admitted, uint4 vectors of bin counters (two grids of nb*nb),
+// middle hits per station kept in shared memory, resident CTAs per SM asked of the compiler
+constexpr int kMaxNbH = 40, kMaxNbM = 20;
+constexpr int kWM = 1, kCapM = 128, kNcvM = (2 * kMaxNbM * kMaxNbM + 3) / 4, kListM = 128, kMinBM = 16;
+constexpr int kWH = 4, kCapH = 448, kNcvH = (2 * kMaxNbH * kMaxNbH + 3) / 4, kListH = 64, kMinBH = 8;
+constexpr int kWG = 16, kCapG = 4096, kNcvG = kNcvH, kListG = 512, kMinBG = 1;
+using SmemM = TeamSmem<kWM, kCapM, kNcvM, kListM>;
+using SmemH = TeamSmem<kWH, kCapH, kNcvH, kListH>;
+using SmemG = TeamSmem<kWG, kCapG, kNcvG, kListG>;
+#define TEAM_KERNEL_M team_kernel<kWM, kCapM, kNcvM, kListM, kClsM, kMinBM>
+#define TEAM_KERNEL_H team_kernel<kWH, kCapH, kNcvH, kListH, kClsH, kMinBH>
+#define TEAM_KERNEL_G team_kernel<kWG, kCapG, kNcvG, kListG, kClsG, kMinBG>
 
 enum SlotState { kEmpty = 0, kUploaded = 1, kRunning = 2 };
 
 struct Scratch {
   Ctrl* d_ctrl = nullptr;
   uint32_t* d_list[kNumTeamClasses] = {nullptr, nullptr, nullptr};
+  uint32_t* d_spill[kNumTeamClasses] = {nullptr, nullptr, nullptr};  // per CTA: middle-hit lists beyond shared memory
 };
 
 struct ProfEvents {
@@ -174,7 +180,7 @@ int build_params(const cbm_trigger_config_t& c, Params& p, std::string& why) {
     const int half = (int)std::ceil(smax * K);
     p.key_min = -half;
     int shH = sh;
-    while (((2 * half) >> shH) + 1 > 48) ++shH;
+    while (((2 * half) >> shH) + 1 > kMaxNbH) ++shH;
     p.cls_shift[kClsH] = p.cls_shift[kClsG] = shH;
     p.cls_nb[kClsH] = p.cls_nb[kClsG] = (uint32_t)(((2 * half) >> shH) + 1);
     p.cls_shift[kClsM] = shH + 1;
@@ -187,7 +193,7 @@ int build_params(const cbm_trigger_config_t& c, Params& p, std::string& why) {
     if (mi < 0 || mi > 0x7FFFFFFFll) { why = "internal: key multiplier out of range"; return CBM_ERR_INVALID_ARG; }
     p.key_mul[l] = (int32_t)mi;
   }
-  if (p.cls_nb[kClsM] * p.cls_nb[kClsM] > (uint32_t)kNcM || p.cls_nb[kClsH] * p.cls_nb[kClsH] > (uint32_t)kNcH) {
+  if (p.cls_nb[kClsM] > (uint32_t)kMaxNbM || p.cls_nb[kClsH] > (uint32_t)kMaxNbH) {
     why = "internal: bin grid too large";
     return CBM_ERR_INVALID_ARG;
   }
@@ -197,12 +203,16 @@ int build_params(const cbm_trigger_config_t& c, Params& p, std::string& why) {
 // ---------------------------------------------------------------------------------------------- allocation
 int alloc_scratch(cbm_trigger* h, Scratch& s) {
   CBM_CUDA(h, cudaMalloc(&s.d_ctrl, sizeof(Ctrl)));
-  for (int c = 0; c < kNumTeamClasses; ++c) CBM_CUDA(h, cudaMalloc(&s.d_list[c], (size_t)h->cfg.max_events * sizeof(uint32_t)));
+  const size_t cap[kNumTeamClasses] = {kCapM, kCapH, kCapG};
+  for (int c = 0; c < kNumTeamClasses; ++c) {
+    CBM_CUDA(h, cudaMalloc(&s.d_list[c], (size_t)h->cfg.max_events * sizeof(uint32_t)));
+    CBM_CUDA(h, cudaMalloc(&s.d_spill[c], (size_t)h->grid[c] * 6 * cap[c] * sizeof(uint32_t)));
+  }
   return CBM_OK;
 }
 void free_scratch(Scratch& s) {
   cudaFree(s.d_ctrl);
-  for (int c = 0; c < kNumTeamClasses; ++c) cudaFree(s.d_list[c]);
+  for (int c = 0; c < kNumTeamClasses; ++c) { cudaFree(s.d_list[c]); cudaFree(s.d_spill[c]); }
   s = Scratch();
 }
 int make_prof(cbm_trigger* h, ProfEvents& pe) {
@@ -273,14 +283,14 @@ int launch_selection(cbm_trigger* h, const Scratch& scr, const int32_t* d_x, con
   tile_kernel<<<n_tiles, kTileEvents * p.S, 0, st>>>(p, d_x, d_y, d_off, n_events, (uint32_t)n_hits, d_nt, d_nc, d_ac,
                                                      scr.d_ctrl, scr.d_list[kClsM], scr.d_list[kClsH], scr.d_list[kClsG]);
   if (prof) CBM_CUDA(h, cudaEventRecord(prof->k[1], st));
-  team_kernel<kWM, kCapM, kNcM, kClsM><<<h->grid[kClsM], 32 * kWM, sizeof(SmemM), st>>>(
-      p, d_x, d_y, d_off, d_nt, d_nc, d_ac, scr.d_ctrl, scr.d_list[kClsM]);
+  TEAM_KERNEL_M<<<h->grid[kClsM], 32 * kWM, sizeof(SmemM), st>>>(
+      p, d_x, d_y, d_off, d_nt, d_nc, d_ac, scr.d_ctrl, scr.d_list[kClsM], scr.d_spill[kClsM]);
   if (prof) CBM_CUDA(h, cudaEventRecord(prof->k[2], st));
-  team_kernel<kWH, kCapH, kNcH, kClsH><<<h->grid[kClsH], 32 * kWH, sizeof(SmemH), st>>>(
-      p, d_x, d_y, d_off, d_nt, d_nc, d_ac, scr.d_ctrl, scr.d_list[kClsH]);
+  TEAM_KERNEL_H<<<h->grid[kClsH], 32 * kWH, sizeof(SmemH), st>>>(
+      p, d_x, d_y, d_off, d_nt, d_nc, d_ac, scr.d_ctrl, scr.d_list[kClsH], scr.d_spill[kClsH]);
   if (prof) CBM_CUDA(h, cudaEventRecord(prof->k[3], st));
-  team_kernel<kWG, kCapG, kNcG, kClsG><<<h->grid[kClsG], 32 * kWG, sizeof(SmemG), st>>>(
-      p, d_x, d_y, d_off, d_nt, d_nc, d_ac, scr.d_ctrl, scr.d_list[kClsG]);
+  TEAM_KERNEL_G<<<h->grid[kClsG], 32 * kWG, sizeof(SmemG), st>>>(
+      p, d_x, d_y, d_off, d_nt, d_nc, d_ac, scr.d_ctrl, scr.d_list[kClsG], scr.d_spill[kClsG]);
   if (prof) { CBM_CUDA(h, cudaEventRecord(prof->k[4], st)); prof->valid = true; }
   CBM_CUDA(h, cudaGetLastError());
   return 4;
@@ -363,9 +373,9 @@ int cbm_trigger_create(const cbm_trigger_config_t* cfg, cbm_trigger_t** out) {
   CREATE_CUDA(cudaGetDeviceProperties(&prop, cfg->device));
   if (prop.major < 10) { fail(h, CBM_ERR_CUDA, "device is sm_%d%d; this library holds sm_100a code only", prop.major, prop.minor); return bail(CBM_ERR_CUDA); }
   h->n_sm = prop.multiProcessorCount;
-  CREATE_TRY(occupancy_grid(h, team_kernel<kWM, kCapM, kNcM, kClsM>, 32 * kWM, sizeof(SmemM), &h->grid[kClsM]));
-  CREATE_TRY(occupancy_grid(h, team_kernel<kWH, kCapH, kNcH, kClsH>, 32 * kWH, sizeof(SmemH), &h->grid[kClsH]));
-  CREATE_TRY(occupancy_grid(h, team_kernel<kWG, kCapG, kNcG, kClsG>, 32 * kWG, sizeof(SmemG), &h->grid[kClsG]));
+  CREATE_TRY(occupancy_grid(h, TEAM_KERNEL_M, 32 * kWM, sizeof(SmemM), &h->grid[kClsM]));
+  CREATE_TRY(occupancy_grid(h, TEAM_KERNEL_H, 32 * kWH, sizeof(SmemH), &h->grid[kClsH]));
+  CREATE_TRY(occupancy_grid(h, TEAM_KERNEL_G, 32 * kWG, sizeof(SmemG), &h->grid[kClsG]));
   CREATE_CUDA(cudaStreamCreateWithFlags(&h->st_h2d, cudaStreamNonBlocking));
   CREATE_CUDA(cudaStreamCreateWithFlags(&h->st_run, cudaStreamNonBlocking));
   CREATE_CUDA(cudaStreamCreateWithFlags(&h->st_d2h, cudaStreamNonBlocking));

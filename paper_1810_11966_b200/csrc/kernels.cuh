@@ -243,55 +243,65 @@ __global__ void __launch_bounds__(kTileEvents* kMaxStations)
 
 // ================================================================================================ team kernel
 // One team = one CTA of W warps works on one event at a time (persistent: events are fetched from the class
-// list with an atomic cursor).  CAP = fullest layer the class admits, NC >= nb*nb cells per binned layer.
+// list with an atomic cursor, two fetches ahead so that the next event can be prefetched into L2).
+// CAP = fullest layer the class admits; NCV = uint4 vectors of bin counters (both binned layers of a station);
+// LISTCAP = middle hits with triplets kept in shared memory per station (more spill to a global scratch).
 template <int W>
 __device__ __forceinline__ void team_sync() {
   if (W == 1) __syncwarp(); else __syncthreads();
 }
 
-template <int W, int CAP, int NC>
+template <int W, int CAP, int NCV, int LISTCAP>
 struct TeamSmem {
-  int32_t sx0[CAP], sy0[CAP];      // layer 0 of the station, bin-sorted
-  int32_t sx2[CAP], sy2[CAP];      // layer 2, bin-sorted
-  uint32_t m[CAP];                 // m[i1] = number of triplets with middle hit i1   (R8: linking sees only h1)
-  int32_t ux[2][CAP], uy[2][CAP];  // distinct middle hits with m > 0 of the previous / current station
-  uint32_t uc[2][CAP];             // their saturated chain counts c_s[u]
-  uint32_t cell0[NC + 1], cell2[NC + 1];  // cell c of the layer = [cell[c], cell[c+1])
-  uint32_t queue[W][64];           // per-warp queue of compatible (h0,h1) pairs: (i0_sorted << 16) | i1
+  alignas(16) uint32_t cellraw[4 + 4 * NCV];  // cell = cellraw + 4: cell[k] = end of bin k after the scatter, cell[-1] = 0
+  int32_t sx[2 * CAP], sy[2 * CAP];           // layer 0 then layer 2 of the station, bin-sorted
+  uint32_t m[CAP];                            // m[i1] = number of triplets with middle hit i1   (R8)
+  int32_t ux[2][LISTCAP], uy[2][LISTCAP];     // distinct middle hits with m > 0 of the previous / current station
+  uint32_t uc[2][LISTCAP];                    // their saturated chain counts c_s[u]
+  uint32_t queue[W][64];                      // per-warp queue of compatible (h0,h1) pairs: (j_sorted << 16) | i1
+  uint16_t cid[2 * CAP];                      // bin of every hit of layers 0 and 2 (count pass -> scatter pass)
   uint32_t off[kMaxLayers + 1];
   uint32_t wsum[32];
-  unsigned long long acc;          // block-wide u64 accumulator (triplet total / candidate total)
+  unsigned long long acc;                     // block-wide u64 accumulator (triplet total / candidate total)
   uint32_t ucount;
-  uint32_t ev;
+  uint32_t li[3];                             // ring of fetched work indices
 };
 
-// in-place exclusive scan of a[1..n] (a[0] stays 0) by the whole team
+// in-place exclusive scan of cell[0 .. 4*nvec) by the whole team, 128-bit shared-memory accesses
 template <int W>
-__device__ __forceinline__ void team_exclusive_scan(uint32_t* a, uint32_t n, uint32_t* wsum) {
+__device__ __forceinline__ void team_exclusive_scan(uint32_t* cell, uint32_t nvec, uint32_t* wsum) {
   constexpr uint32_t T = 32 * W;
   const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const uint32_t chunk = (n + T - 1) / T;
-  const uint32_t lo = min(tid * chunk, n), hi = min(lo + chunk, n);
+  const uint32_t chunk = (nvec + T - 1) / T;
+  const uint32_t lo = min(tid * chunk, nvec), hi = min(lo + chunk, nvec);
+  uint4* const v = reinterpret_cast<uint4*>(cell);
   uint32_t sum = 0;
-  for (uint32_t i = lo; i < hi; ++i) sum += a[1 + i];
+  for (uint32_t i = lo; i < hi; ++i) {
+    const uint4 c = v[i];
+    sum += c.x + c.y + c.z + c.w;
+  }
   uint32_t incl = sum;
 #pragma unroll
   for (int d = 1; d < 32; d <<= 1) {
-    const uint32_t v = __shfl_up_sync(0xFFFFFFFFu, incl, d);
-    if (lane >= (uint32_t)d) incl += v;
+    const uint32_t u = __shfl_up_sync(0xFFFFFFFFu, incl, d);
+    if (lane >= (uint32_t)d) incl += u;
   }
   uint32_t base = incl - sum;
   if (W > 1) {
     if (lane == 31) wsum[warp] = incl;
     __syncthreads();
-    uint32_t wbase = 0;
-    for (uint32_t w = 0; w < warp; ++w) wbase += wsum[w];
-    base += wbase;
+    uint32_t wv = lane < (uint32_t)W ? wsum[lane] : 0u;
+    if (lane >= warp) wv = 0;
+#pragma unroll
+    for (int d = 16; d >= 1; d >>= 1) wv += __shfl_xor_sync(0xFFFFFFFFu, wv, d);
+    base += wv;
   }
   for (uint32_t i = lo; i < hi; ++i) {
-    const uint32_t c = a[1 + i];
-    a[1 + i] = base;
-    base += c;
+    const uint4 c = v[i];
+    uint4 o;
+    o.x = base; o.y = o.x + c.x; o.z = o.y + c.y; o.w = o.z + c.z;
+    base = o.w + c.w;
+    v[i] = o;
   }
 }
 
@@ -299,36 +309,52 @@ __device__ __forceinline__ int bin_of(int key, int kmin, int sh, int nbm1) {
   return min(max((key - kmin) >> sh, 0), nbm1);
 }
 
-// Phase 2 (a5): for one compatible (h0,h1) pair, count the h2 of layer 2 compatible with both.
-// Looks only at the 2-D bins around h1's slope (superset of its window), tests exactly.
-template <class SM>
-__device__ __forceinline__ uint32_t count_h2(const SM& sm, int32_t x0, int32_t y0, int32_t x1, int32_t y1, int32_t z0,
-                                             int32_t z1, int32_t z2, int64_t T02, int64_t T12, int32_t M1, int kmin,
-                                             int R, int sh, int nb) {
-  const int kx = __mulhi(x1, M1), ky = __mulhi(y1, M1);
+__device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+
+// The bins that can hold a hit compatible with a hit of slope keys (kx, ky): at most two rows (bx) of
+// consecutive bins, because 2*R <= 2^shift.  Rows as index ranges [a0,e0), [a1,e1) of a bin-sorted layer
+// whose bins start at cell[base].
+struct Rows { uint32_t a0, n0, a1, n1; };
+__device__ __forceinline__ Rows rows_of(const uint32_t* cell, int base, int kx, int ky, int kmin, int R, int sh, int nb) {
   const int bxl = bin_of(kx - R, kmin, sh, nb - 1), bxh = bin_of(kx + R, kmin, sh, nb - 1);
   const int byl = bin_of(ky - R, kmin, sh, nb - 1), byh = bin_of(ky + R, kmin, sh, nb - 1);
+  const int r0 = base + bxl * nb, r1 = base + bxh * nb;
+  Rows r;
+  r.a0 = cell[r0 + byl - 1];
+  r.n0 = cell[r0 + byh] - r.a0;
+  r.a1 = cell[r1 + byl - 1];
+  r.n1 = bxh != bxl ? cell[r1 + byh] - r.a1 : 0u;
+  return r;
+}
+
+// Phase 2 (a5): for one compatible (h0,h1) pair, count the h2 of layer 2 compatible with both.
+// Looks only at the 2-D bins around h1's slope (superset of its window), tests exactly.
+__device__ __forceinline__ uint32_t count_h2(const uint32_t* cell, const int32_t* sx, const int32_t* sy, int base2,
+                                             int32_t x0, int32_t y0, int32_t x1, int32_t y1, int32_t z0, int32_t z1,
+                                             int32_t z2, int64_t T02, int64_t T12, int32_t M1, int kmin, int R, int sh,
+                                             int nb) {
+  const Rows r = rows_of(cell, base2, __mulhi(x1, M1), __mulhi(y1, M1), kmin, R, sh, nb);
   const int64_t Qx0 = (int64_t)x0 * z2 + T02, Qy0 = (int64_t)y0 * z2 + T02;
   const int64_t Qx1 = (int64_t)x1 * z2 + T12, Qy1 = (int64_t)y1 * z2 + T12;
   uint32_t c = 0;
-  for (int bx = bxl; bx <= bxh; ++bx) {
-    const uint32_t ja = sm.cell2[bx * nb + byl], jb = sm.cell2[bx * nb + byh + 1];
-    for (uint32_t j = ja; j < jb; ++j) {
-      const int32_t x2 = sm.sx2[j], y2 = sm.sy2[j];
-      const bool ok = win(Qx1, x2, z1, 2 * (uint64_t)T12) & win(Qy1, y2, z1, 2 * (uint64_t)T12) &
-                      win(Qx0, x2, z0, 2 * (uint64_t)T02) & win(Qy0, y2, z0, 2 * (uint64_t)T02);
-      c += ok ? 1u : 0u;
-    }
+  const uint32_t n = r.n0 + r.n1;
+  for (uint32_t k = 0; k < n; ++k) {
+    const uint32_t j = k < r.n0 ? r.a0 + k : r.a1 + (k - r.n0);
+    const int32_t x2 = sx[j], y2 = sy[j];
+    const bool ok = win(Qx1, x2, z1, 2 * (uint64_t)T12) & win(Qy1, y2, z1, 2 * (uint64_t)T12) &
+                    win(Qx0, x2, z0, 2 * (uint64_t)T02) & win(Qy0, y2, z0, 2 * (uint64_t)T02);
+    c += ok ? 1u : 0u;
   }
   return c;
 }
 
-template <int W, int CAP, int NC, int CLS>
-__global__ void __launch_bounds__(32 * W)
+template <int W, int CAP, int NCV, int LISTCAP, int CLS, int MINB>
+__global__ void __launch_bounds__(32 * W, MINB)
     team_kernel(const __grid_constant__ Params p, const int32_t* __restrict__ x, const int32_t* __restrict__ y,
                 const uint32_t* __restrict__ off, uint32_t* __restrict__ n_triplets, uint32_t* __restrict__ n_candidates,
-                uint8_t* __restrict__ accept, Ctrl* __restrict__ ctrl, const uint32_t* __restrict__ list) {
-  using SM = TeamSmem<W, CAP, NC>;
+                uint8_t* __restrict__ accept, Ctrl* __restrict__ ctrl, const uint32_t* __restrict__ list,
+                uint32_t* __restrict__ spill) {
+  using SM = TeamSmem<W, CAP, NCV, LISTCAP>;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   SM& sm = *reinterpret_cast<SM*>(smem_raw);
   constexpr uint32_t T = 32 * W;
@@ -336,14 +362,41 @@ __global__ void __launch_bounds__(32 * W)
   const uint32_t S = p.S, L = p.L;
   const uint32_t n_list = ctrl->count[CLS];
   const int kmin = p.key_min, R = p.key_R, sh = p.cls_shift[CLS], nb = (int)p.cls_nb[CLS];
-  const uint32_t ncell = (uint32_t)(nb * nb);
+  const int ncell = nb * nb;
+  const uint32_t nvec = (uint32_t)(2 * ncell + 3) >> 2;
+  uint32_t* const cell = sm.cellraw + 4;
+  // spill area of this CTA: lists beyond LISTCAP entries, [2][3][CAP] words (x, y, c)
+  uint32_t* const spill_cta = spill + (size_t)blockIdx.x * 6 * CAP;
+  auto list_x = [&](int which, uint32_t i) -> int32_t& {
+    return i < (uint32_t)LISTCAP ? sm.ux[which][i] : reinterpret_cast<int32_t*>(spill_cta)[(which * 3 + 0) * CAP + (i - LISTCAP)];
+  };
+  auto list_y = [&](int which, uint32_t i) -> int32_t& {
+    return i < (uint32_t)LISTCAP ? sm.uy[which][i] : reinterpret_cast<int32_t*>(spill_cta)[(which * 3 + 1) * CAP + (i - LISTCAP)];
+  };
+  auto list_c = [&](int which, uint32_t i) -> uint32_t& {
+    return i < (uint32_t)LISTCAP ? sm.uc[which][i] : spill_cta[(which * 3 + 2) * CAP + (i - LISTCAP)];
+  };
 
-  for (;;) {
-    if (tid == 0) sm.ev = atomicAdd(&ctrl->work[CLS], 1u);
-    team_sync<W>();
-    const uint32_t li = sm.ev;
+  if (tid == 0) {
+    sm.li[0] = atomicAdd(&ctrl->work[CLS], 1u);
+    sm.li[1] = atomicAdd(&ctrl->work[CLS], 1u);
+    sm.cellraw[3] = 0;
+  }
+  team_sync<W>();
+
+  for (uint32_t it3 = 0;; it3 = it3 == 2 ? 0 : it3 + 1) {
+    const uint32_t li = sm.li[it3];
     if (li >= n_list) break;
-    const uint32_t e = list[li];
+    const uint32_t nxt = sm.li[it3 == 2 ? 0 : it3 + 1];
+    if (tid == 0) sm.li[it3 == 0 ? 2 : it3 - 1] = atomicAdd(&ctrl->work[CLS], 1u);
+    const uint32_t e = __ldg(list + li);
+    // extent of the NEXT event: loaded now, used for its L2 prefetch after station 0 (latency hidden)
+    uint32_t pf_a = 0, pf_b = 0;
+    if (nxt < n_list) {
+      const uint32_t e2 = __ldg(list + nxt);
+      pf_a = __ldg(off + (size_t)e2 * L);
+      pf_b = __ldg(off + (size_t)e2 * L + L);
+    }
     for (uint32_t i = tid; i <= L; i += T) sm.off[i] = __ldg(off + (size_t)e * L + i);
     team_sync<W>();
 
@@ -357,38 +410,34 @@ __global__ void __launch_bounds__(32 * W)
       const int32_t M0 = p.key_mul[3 * s], M1 = p.key_mul[3 * s + 1], M2 = p.key_mul[3 * s + 2];
       const int64_t T01 = p.thr_in[s][0], T02 = p.thr_in[s][1], T12 = p.thr_in[s][2];
       if (tid == 0) { sm.acc = 0; sm.ucount = 0; }
-      bool any_triplet_possible = (n0 != 0) & (n1 != 0) & (n2 != 0);
-      if (any_triplet_possible) {
-        // ---- a4: bin layers 0 and 2 on a 2-D slope grid (count, scan, scatter)
-        for (uint32_t i = tid; i <= ncell; i += T) { sm.cell0[i] = 0; sm.cell2[i] = 0; }
-        for (uint32_t i = tid; i < n1; i += T) sm.m[i] = 0;
-        team_sync<W>();
-        for (uint32_t i = tid; i < n0 + n2; i += T) {
-          const bool l2 = i >= n0;
-          const uint32_t g = l2 ? b2 + (i - n0) : b0 + i;
-          const int32_t hx = __ldg(x + g), hy = __ldg(y + g);
-          const int32_t M = l2 ? M2 : M0;
-          const int c = bin_of(__mulhi(hx, M), kmin, sh, nb - 1) * nb + bin_of(__mulhi(hy, M), kmin, sh, nb - 1);
-          atomicAdd(l2 ? &sm.cell2[c + 1] : &sm.cell0[c + 1], 1u);
+      const bool search = (n0 != 0) & (n1 != 0) & (n2 != 0);
+      if (search) {
+        // ---- a4: bin layers 0 and 2 on a 2-D slope grid: count, one scan over both grids, scatter
+        {
+          uint4* const v = reinterpret_cast<uint4*>(cell);
+          for (uint32_t i = tid; i < nvec; i += T) v[i] = make_uint4(0, 0, 0, 0);
+          for (uint32_t i = tid; i < n1; i += T) sm.m[i] = 0;
         }
         team_sync<W>();
-        team_exclusive_scan<W>(sm.cell0, ncell, sm.wsum);
-        team_sync<W>();
-        team_exclusive_scan<W>(sm.cell2, ncell, sm.wsum);
-        team_sync<W>();
         for (uint32_t i = tid; i < n0 + n2; i += T) {
           const bool l2 = i >= n0;
           const uint32_t g = l2 ? b2 + (i - n0) : b0 + i;
           const int32_t hx = __ldg(x + g), hy = __ldg(y + g);
           const int32_t M = l2 ? M2 : M0;
-          const int c = bin_of(__mulhi(hx, M), kmin, sh, nb - 1) * nb + bin_of(__mulhi(hy, M), kmin, sh, nb - 1);
-          if (l2) {
-            const uint32_t pos = atomicAdd(&sm.cell2[c + 1], 1u);
-            sm.sx2[pos] = hx; sm.sy2[pos] = hy;
-          } else {
-            const uint32_t pos = atomicAdd(&sm.cell0[c + 1], 1u);
-            sm.sx0[pos] = hx; sm.sy0[pos] = hy;
-          }
+          const int c = (l2 ? ncell : 0) + bin_of(__mulhi(hx, M), kmin, sh, nb - 1) * nb +
+                        bin_of(__mulhi(hy, M), kmin, sh, nb - 1);
+          sm.cid[i] = (uint16_t)c;
+          atomicAdd(&cell[c], 1u);
+        }
+        team_sync<W>();
+        team_exclusive_scan<W>(cell, nvec, sm.wsum);
+        team_sync<W>();
+        for (uint32_t i = tid; i < n0 + n2; i += T) {
+          const uint32_t g = i >= n0 ? b2 + (i - n0) : b0 + i;
+          const int32_t hx = __ldg(x + g), hy = __ldg(y + g);  // L1 hit
+          const uint32_t pos = atomicAdd(&cell[sm.cid[i]], 1u);
+          sm.sx[pos] = hx;
+          sm.sy[pos] = hy;
         }
         team_sync<W>();
 
@@ -400,33 +449,23 @@ __global__ void __launch_bounds__(32 * W)
           const uint32_t i1 = base + lane;
           const bool act = i1 < n1;
           int32_t x1 = 0, y1 = 0;
-          int bx = 0, bxh = -1, byl = 0, byh = 0;
-          uint32_t j = 0, jend = 0;
+          Rows r = {0, 0, 0, 0};
           if (act) {
-            x1 = __ldg(x + b1 + i1); y1 = __ldg(y + b1 + i1);
-            const int kx = __mulhi(x1, M1), ky = __mulhi(y1, M1);
-            bx = bin_of(kx - R, kmin, sh, nb - 1) - 1;  // advanced to the first row below
-            bxh = bin_of(kx + R, kmin, sh, nb - 1);
-            byl = bin_of(ky - R, kmin, sh, nb - 1);
-            byh = bin_of(ky + R, kmin, sh, nb - 1);
+            x1 = __ldg(x + b1 + i1);
+            y1 = __ldg(y + b1 + i1);
+            r = rows_of(cell, 0, __mulhi(x1, M1), __mulhi(y1, M1), kmin, R, sh, nb);
           }
+          const uint32_t nc = r.n0 + r.n1;
+          const uint32_t ncmax = __reduce_max_sync(0xFFFFFFFFu, nc);
           // |x0*z1 - x1*z0| <= T01  <=>  (uint64)(x0*z1 + (T01 - x1*z0)) <= 2*T01
           const int64_t Qx = T01 - (int64_t)x1 * z0, Qy = T01 - (int64_t)y1 * z0;
-          for (;;) {
-            if (j >= jend && bx < bxh) {  // next row of bins
-              ++bx;
-              j = sm.cell0[bx * nb + byl];
-              jend = sm.cell0[bx * nb + byh + 1];
-            }
-            const bool more = (j < jend) | (bx < bxh);
-            if (!__any_sync(0xFFFFFFFFu, more)) break;
+          for (uint32_t k = 0; k < ncmax; ++k) {
+            const uint32_t j = k < r.n0 ? r.a0 + k : r.a1 + (k - r.n0);
             bool pass = false;
-            if (j < jend) {
-              const int32_t hx = sm.sx0[j];
-              if ((uint64_t)((int64_t)hx * z1 + Qx) <= 2 * (uint64_t)T01) {
-                const int32_t hy = sm.sy0[j];
-                pass = (uint64_t)((int64_t)hy * z1 + Qy) <= 2 * (uint64_t)T01;
-              }
+            if (k < nc) {
+              const int32_t hx = sm.sx[j], hy = sm.sy[j];
+              pass = ((uint64_t)((int64_t)hx * z1 + Qx) <= 2 * (uint64_t)T01) &
+                     ((uint64_t)((int64_t)hy * z1 + Qy) <= 2 * (uint64_t)T01);
             }
             const uint32_t pm = __ballot_sync(0xFFFFFFFFu, pass);
             if (pm) {
@@ -437,37 +476,43 @@ __global__ void __launch_bounds__(32 * W)
                 qn -= 32;
                 const uint32_t ent = q[qn + lane];
                 const uint32_t j0 = ent >> 16, k1 = ent & 0xFFFFu;
-                const uint32_t c = count_h2(sm, sm.sx0[j0], sm.sy0[j0], __ldg(x + b1 + k1), __ldg(y + b1 + k1), z0, z1,
-                                            z2, T02, T12, M1, kmin, R, sh, nb);
+                const uint32_t c = count_h2(cell, sm.sx, sm.sy, ncell, sm.sx[j0], sm.sy[j0], __ldg(x + b1 + k1),
+                                            __ldg(y + b1 + k1), z0, z1, z2, T02, T12, M1, kmin, R, sh, nb);
                 if (c) atomicAdd(&sm.m[k1], c);
                 __syncwarp();
               }
             }
-            if (j < jend) ++j;
           }
         }
         __syncwarp();
         if (lane < qn) {
           const uint32_t ent = q[lane];
           const uint32_t j0 = ent >> 16, k1 = ent & 0xFFFFu;
-          const uint32_t c = count_h2(sm, sm.sx0[j0], sm.sy0[j0], __ldg(x + b1 + k1), __ldg(y + b1 + k1), z0, z1, z2,
-                                      T02, T12, M1, kmin, R, sh, nb);
+          const uint32_t c = count_h2(cell, sm.sx, sm.sy, ncell, sm.sx[j0], sm.sy[j0], __ldg(x + b1 + k1),
+                                      __ldg(y + b1 + k1), z0, z1, z2, T02, T12, M1, kmin, R, sh, nb);
           if (c) atomicAdd(&sm.m[k1], c);
+        }
+      }
+      if (s == 0 && pf_b > pf_a) {  // pull the next event of this team into L2 while this one is being searched
+        const uint32_t la = pf_a >> 5, lb = (pf_b + 31) >> 5;  // 128-byte lines
+        for (uint32_t l = la + tid; l < lb; l += T) {
+          prefetch_l2(x + (size_t)l * 32);
+          prefetch_l2(y + (size_t)l * 32);
         }
       }
       team_sync<W>();
 
       // ---- station total, list of distinct middle hits with triplets (R8)
-      if (any_triplet_possible) {
+      if (search) {
         unsigned long long part = 0;
         for (uint32_t i = tid; i < n1; i += T) {
           const uint32_t mm = sm.m[i];
           part += mm;
           if (mm && !dead) {
             const uint32_t pos = atomicAdd(&sm.ucount, 1u);
-            sm.ux[cur][pos] = __ldg(x + b1 + i);
-            sm.uy[cur][pos] = __ldg(y + b1 + i);
-            sm.uc[cur][pos] = mm;
+            list_x(cur, pos) = __ldg(x + b1 + i);
+            list_y(cur, pos) = __ldg(y + b1 + i);
+            list_c(cur, pos) = mm;
           }
         }
 #pragma unroll
@@ -482,17 +527,17 @@ __global__ void __launch_bounds__(32 * W)
         const int32_t zA = p.z[3 * (s - 1) + 1], zB = z1;
         const int64_t TL = p.thr_link[s];
         for (uint32_t u = tid; u < ncur; u += T) {
-          const int32_t xu = sm.ux[cur][u], yu = sm.uy[cur][u];
+          const int32_t xu = list_x(cur, u), yu = list_y(cur, u);
           // |x_t*zB - x_u*zA| <= TL
           const int64_t Qx = TL - (int64_t)xu * zA, Qy = TL - (int64_t)yu * zA;
           unsigned long long a = 0;
           for (uint32_t t = 0; t < nprev; ++t) {
-            const bool ok = ((uint64_t)((int64_t)sm.ux[cur ^ 1][t] * zB + Qx) <= 2 * (uint64_t)TL) &
-                            ((uint64_t)((int64_t)sm.uy[cur ^ 1][t] * zB + Qy) <= 2 * (uint64_t)TL);
-            if (ok) a += sm.uc[cur ^ 1][t];  // < 4096 * 2^32
+            const bool ok = ((uint64_t)((int64_t)list_x(cur ^ 1, t) * zB + Qx) <= 2 * (uint64_t)TL) &
+                            ((uint64_t)((int64_t)list_y(cur ^ 1, t) * zB + Qy) <= 2 * (uint64_t)TL);
+            if (ok) a += list_c(cur ^ 1, t);  // < 4096 * 2^32
           }
           a = sat32(a);
-          sm.uc[cur][u] = sat32(a * (unsigned long long)sm.uc[cur][u]);  // m_u <= 2^24: no overflow
+          list_c(cur, u) = sat32(a * (unsigned long long)list_c(cur, u));  // m_u <= 2^24: no overflow
         }
       }
       if (ncur == 0) dead = true;
@@ -506,7 +551,7 @@ __global__ void __launch_bounds__(32 * W)
     team_sync<W>();
     if (!dead) {
       unsigned long long part = 0;
-      for (uint32_t u = tid; u < nprev; u += T) part += sm.uc[cur ^ 1][u];
+      for (uint32_t u = tid; u < nprev; u += T) part += list_c(cur ^ 1, u);
 #pragma unroll
       for (int d = 16; d >= 1; d >>= 1) part += __shfl_xor_sync(0xFFFFFFFFu, part, d);
       if (lane == 0 && part) atomicAdd(&sm.acc, part);

@@ -139,7 +139,7 @@ def test_layers_up_to_max_hits_per_layer():
     z = list(W.GEOMETRY_4)
     ev = [big_uniform_event(z, [4096, 700, 900, 300, 4096, 300, 600, 600, 4096, 1500, 1500, 1500], rng),
           big_uniform_event(z, [129] * 12, rng), big_uniform_event(z, [128] * 12, rng),
-          big_uniform_event(z, [513] + [40] * 11, rng), big_uniform_event(z, [512] * 12, rng),
+          big_uniform_event(z, [449] + [40] * 11, rng), big_uniform_event(z, [448] * 12, rng),
           big_uniform_event(z, [25] * 12, rng), big_uniform_event(z, [24] * 12, rng)]
     x, y, off = W.batch_from_layers(z, ev)
     got = gpu_select(z, x, y, off)
