@@ -30,9 +30,9 @@ constexpr int kWG = 16, kCapG = 4096, kNcvG = kNcvH, kListG = 512, kMinBG = 1;
 using SmemM = TeamSmem<kWM, kCapM, kNcvM, kListM>;
 using SmemH = TeamSmem<kWH, kCapH, kNcvH, kListH>;
 using SmemG = TeamSmem<kWG, kCapG, kNcvG, kListG>;
-#define TEAM_KERNEL_M team_kernel<kWM, kCapM, kNcvM, kListM, kClsM, kMinBM>
-#define TEAM_KERNEL_H team_kernel<kWH, kCapH, kNcvH, kListH, kClsH, kMinBH>
-#define TEAM_KERNEL_G team_kernel<kWG, kCapG, kNcvG, kListG, kClsG, kMinBG>
+#define TEAM_KERNEL_M team_kernel<kWM, kCapM, kNcvM, kListM, kClsM, kMinBM, true>
+#define TEAM_KERNEL_H team_kernel<kWH, kCapH, kNcvH, kListH, kClsH, kMinBH, true>
+#define TEAM_KERNEL_G team_kernel<kWG, kCapG, kNcvG, kListG, kClsG, kMinBG, false>
 
 enum SlotState { kEmpty = 0, kUploaded = 1, kRunning = 2 };
 
@@ -143,7 +143,9 @@ int build_params(const cbm_trigger_config_t& c, Params& p, std::string& why) {
     if (s) {
       const int64_t zA = p.z[3 * (s - 1) + 1];
       p.thr_link[s] = (int64_t)c.win_link_num * zA * z1 / (int64_t)c.win_link_den;
+      p.thr2_link[s] = 2 * (uint64_t)p.thr_link[s];
     }
+    for (int k = 0; k < 3; ++k) p.thr2_in[s][k] = 2 * (uint64_t)p.thr_in[s][k];
   }
   p.min_candidates = c.min_candidates;
   p.max_hits_per_layer = c.max_hits_per_layer;
@@ -283,10 +285,10 @@ int launch_selection(cbm_trigger* h, const Scratch& scr, const int32_t* d_x, con
   tile_kernel<<<n_tiles, kTileEvents * p.S, 0, st>>>(p, d_x, d_y, d_off, n_events, (uint32_t)n_hits, d_nt, d_nc, d_ac,
                                                      scr.d_ctrl, scr.d_list[kClsM], scr.d_list[kClsH], scr.d_list[kClsG]);
   if (prof) CBM_CUDA(h, cudaEventRecord(prof->k[1], st));
-  TEAM_KERNEL_M<<<h->grid[kClsM], 32 * kWM, sizeof(SmemM), st>>>(
+  TEAM_KERNEL_M<<<h->grid[kClsM], 32 * kWM, 0, st>>>(
       p, d_x, d_y, d_off, d_nt, d_nc, d_ac, scr.d_ctrl, scr.d_list[kClsM], scr.d_spill[kClsM]);
   if (prof) CBM_CUDA(h, cudaEventRecord(prof->k[2], st));
-  TEAM_KERNEL_H<<<h->grid[kClsH], 32 * kWH, sizeof(SmemH), st>>>(
+  TEAM_KERNEL_H<<<h->grid[kClsH], 32 * kWH, 0, st>>>(
       p, d_x, d_y, d_off, d_nt, d_nc, d_ac, scr.d_ctrl, scr.d_list[kClsH], scr.d_spill[kClsH]);
   if (prof) CBM_CUDA(h, cudaEventRecord(prof->k[3], st));
   TEAM_KERNEL_G<<<h->grid[kClsG], 32 * kWG, sizeof(SmemG), st>>>(
@@ -324,7 +326,8 @@ void fill_prof(cbm_trigger_stats_t& st, ProfEvents& pe, bool copies) {
 
 template <class K>
 int occupancy_grid(cbm_trigger* h, K kernel, int threads, size_t smem, int* grid) {
-  CBM_CUDA(h, cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  if (smem) CBM_CUDA(h, cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  CBM_CUDA(h, cudaFuncSetAttribute(kernel, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
   int per_sm = 0;
   CBM_CUDA(h, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, threads, smem));
   if (per_sm < 1) return fail(h, CBM_ERR_CUDA, "a team kernel does not fit on this device");
@@ -373,8 +376,9 @@ int cbm_trigger_create(const cbm_trigger_config_t* cfg, cbm_trigger_t** out) {
   CREATE_CUDA(cudaGetDeviceProperties(&prop, cfg->device));
   if (prop.major < 10) { fail(h, CBM_ERR_CUDA, "device is sm_%d%d; this library holds sm_100a code only", prop.major, prop.minor); return bail(CBM_ERR_CUDA); }
   h->n_sm = prop.multiProcessorCount;
-  CREATE_TRY(occupancy_grid(h, TEAM_KERNEL_M, 32 * kWM, sizeof(SmemM), &h->grid[kClsM]));
-  CREATE_TRY(occupancy_grid(h, TEAM_KERNEL_H, 32 * kWH, sizeof(SmemH), &h->grid[kClsH]));
+  static_assert(sizeof(SmemM) <= 48 * 1024 && sizeof(SmemH) <= 48 * 1024, "static shared memory limit");
+  CREATE_TRY(occupancy_grid(h, TEAM_KERNEL_M, 32 * kWM, 0, &h->grid[kClsM]));
+  CREATE_TRY(occupancy_grid(h, TEAM_KERNEL_H, 32 * kWH, 0, &h->grid[kClsH]));
   CREATE_TRY(occupancy_grid(h, TEAM_KERNEL_G, 32 * kWG, sizeof(SmemG), &h->grid[kClsG]));
   CREATE_CUDA(cudaStreamCreateWithFlags(&h->st_h2d, cudaStreamNonBlocking));
   CREATE_CUDA(cudaStreamCreateWithFlags(&h->st_run, cudaStreamNonBlocking));

@@ -290,10 +290,8 @@ __device__ __forceinline__ void team_exclusive_scan(uint32_t* cell, uint32_t nve
   if (W > 1) {
     if (lane == 31) wsum[warp] = incl;
     __syncthreads();
-    uint32_t wv = lane < (uint32_t)W ? wsum[lane] : 0u;
-    if (lane >= warp) wv = 0;
-#pragma unroll
-    for (int d = 16; d >= 1; d >>= 1) wv += __shfl_xor_sync(0xFFFFFFFFu, wv, d);
+    uint32_t wv = (lane < (uint32_t)W && lane < warp) ? wsum[lane] : 0u;
+    wv = __reduce_add_sync(0xFFFFFFFFu, wv);
     base += wv;
   }
   for (uint32_t i = lo; i < hi; ++i) {
@@ -311,13 +309,20 @@ __device__ __forceinline__ int bin_of(int key, int kmin, int sh, int nbm1) {
 
 __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 
+// exact window test with the anchor side hoisted: Q = T - b*z_a (int64), pass <=> (uint64)(a*z_o + Q) <= 2T
+__device__ __forceinline__ int64_t anchor_q(int32_t b, int32_t neg_za, int64_t T) { return (int64_t)b * neg_za + T; }
+__device__ __forceinline__ bool win_q(int32_t a, int32_t zo, int64_t Q, uint64_t T2) {
+  return (uint64_t)((int64_t)a * zo + Q) <= T2;
+}
+
 // The bins that can hold a hit compatible with a hit of slope keys (kx, ky): at most two rows (bx) of
-// consecutive bins, because 2*R <= 2^shift.  Rows as index ranges [a0,e0), [a1,e1) of a bin-sorted layer
-// whose bins start at cell[base].
+// consecutive bins, because 2*R <= 2^shift.  Rows as index ranges [a0, a0+n0), [a1, a1+n1) of the bin-sorted
+// layer whose bins start at cell[base].
 struct Rows { uint32_t a0, n0, a1, n1; };
 __device__ __forceinline__ Rows rows_of(const uint32_t* cell, int base, int kx, int ky, int kmin, int R, int sh, int nb) {
-  const int bxl = bin_of(kx - R, kmin, sh, nb - 1), bxh = bin_of(kx + R, kmin, sh, nb - 1);
-  const int byl = bin_of(ky - R, kmin, sh, nb - 1), byh = bin_of(ky + R, kmin, sh, nb - 1);
+  const int tx = kx - R - kmin, ty = ky - R - kmin;
+  const int bxl = min(max(tx >> sh, 0), nb - 1), bxh = min(max((tx + 2 * R) >> sh, 0), nb - 1);
+  const int byl = min(max(ty >> sh, 0), nb - 1), byh = min(max((ty + 2 * R) >> sh, 0), nb - 1);
   const int r0 = base + bxl * nb, r1 = base + bxh * nb;
   Rows r;
   r.a0 = cell[r0 + byl - 1];
@@ -327,36 +332,47 @@ __device__ __forceinline__ Rows rows_of(const uint32_t* cell, int base, int kx, 
   return r;
 }
 
+// per-station constants, loaded once per station
+struct StationConst {
+  int32_t z0, z1, z2, nz0, nz1, nz2;  // nz = -z
+  int32_t M0, M1, M2;
+  int64_t T01, T02, T12;
+  uint64_t T01x2, T02x2, T12x2;
+};
+
 // Phase 2 (a5): for one compatible (h0,h1) pair, count the h2 of layer 2 compatible with both.
 // Looks only at the 2-D bins around h1's slope (superset of its window), tests exactly.
-__device__ __forceinline__ uint32_t count_h2(const uint32_t* cell, const int32_t* sx, const int32_t* sy, int base2,
-                                             int32_t x0, int32_t y0, int32_t x1, int32_t y1, int32_t z0, int32_t z1,
-                                             int32_t z2, int64_t T02, int64_t T12, int32_t M1, int kmin, int R, int sh,
+template <class SM>
+__device__ __forceinline__ uint32_t count_h2(const SM& sm, const uint32_t* cell, int ncell, const StationConst& c,
+                                             int32_t x0, int32_t y0, int32_t x1, int32_t y1, int kmin, int R, int sh,
                                              int nb) {
-  const Rows r = rows_of(cell, base2, __mulhi(x1, M1), __mulhi(y1, M1), kmin, R, sh, nb);
-  const int64_t Qx0 = (int64_t)x0 * z2 + T02, Qy0 = (int64_t)y0 * z2 + T02;
-  const int64_t Qx1 = (int64_t)x1 * z2 + T12, Qy1 = (int64_t)y1 * z2 + T12;
-  uint32_t c = 0;
+  const Rows r = rows_of(cell, ncell, __mulhi(x1, c.M1), __mulhi(y1, c.M1), kmin, R, sh, nb);
   const uint32_t n = r.n0 + r.n1;
+  if (n == 0) return 0;
+  // |x2*z1 - x1*z2| <= T12 and |x2*z0 - x0*z2| <= T02 (and the same in y)
+  const int64_t Qx1 = anchor_q(x1, c.nz2, c.T12), Qy1 = anchor_q(y1, c.nz2, c.T12);
+  const int64_t Qx0 = anchor_q(x0, c.nz2, c.T02), Qy0 = anchor_q(y0, c.nz2, c.T02);
+  uint32_t cnt = 0;
   for (uint32_t k = 0; k < n; ++k) {
     const uint32_t j = k < r.n0 ? r.a0 + k : r.a1 + (k - r.n0);
-    const int32_t x2 = sx[j], y2 = sy[j];
-    const bool ok = win(Qx1, x2, z1, 2 * (uint64_t)T12) & win(Qy1, y2, z1, 2 * (uint64_t)T12) &
-                    win(Qx0, x2, z0, 2 * (uint64_t)T02) & win(Qy0, y2, z0, 2 * (uint64_t)T02);
-    c += ok ? 1u : 0u;
+    const int32_t x2 = sm.sx[j], y2 = sm.sy[j];
+    const bool ok = win_q(x2, c.z1, Qx1, c.T12x2) & win_q(y2, c.z1, Qy1, c.T12x2) & win_q(x2, c.z0, Qx0, c.T02x2) &
+                    win_q(y2, c.z0, Qy0, c.T02x2);
+    cnt += ok ? 1u : 0u;
   }
-  return c;
+  return cnt;
 }
 
-template <int W, int CAP, int NCV, int LISTCAP, int CLS, int MINB>
+template <int W, int CAP, int NCV, int LISTCAP, int CLS, int MINB, bool STATIC_SMEM>
 __global__ void __launch_bounds__(32 * W, MINB)
     team_kernel(const __grid_constant__ Params p, const int32_t* __restrict__ x, const int32_t* __restrict__ y,
                 const uint32_t* __restrict__ off, uint32_t* __restrict__ n_triplets, uint32_t* __restrict__ n_candidates,
                 uint8_t* __restrict__ accept, Ctrl* __restrict__ ctrl, const uint32_t* __restrict__ list,
                 uint32_t* __restrict__ spill) {
   using SM = TeamSmem<W, CAP, NCV, LISTCAP>;
-  extern __shared__ __align__(16) unsigned char smem_raw[];
-  SM& sm = *reinterpret_cast<SM*>(smem_raw);
+  extern __shared__ __align__(16) unsigned char smem_dyn[];
+  __shared__ __align__(16) unsigned char smem_static[STATIC_SMEM ? sizeof(SM) : 16];
+  SM& sm = *reinterpret_cast<SM*>(STATIC_SMEM ? smem_static : smem_dyn);
   constexpr uint32_t T = 32 * W;
   const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const uint32_t S = p.S, L = p.L;
@@ -365,17 +381,9 @@ __global__ void __launch_bounds__(32 * W, MINB)
   const int ncell = nb * nb;
   const uint32_t nvec = (uint32_t)(2 * ncell + 3) >> 2;
   uint32_t* const cell = sm.cellraw + 4;
-  // spill area of this CTA: lists beyond LISTCAP entries, [2][3][CAP] words (x, y, c)
+  // spill area of this CTA: list entries beyond LISTCAP, [2 lists][x, y, c][CAP] words
   uint32_t* const spill_cta = spill + (size_t)blockIdx.x * 6 * CAP;
-  auto list_x = [&](int which, uint32_t i) -> int32_t& {
-    return i < (uint32_t)LISTCAP ? sm.ux[which][i] : reinterpret_cast<int32_t*>(spill_cta)[(which * 3 + 0) * CAP + (i - LISTCAP)];
-  };
-  auto list_y = [&](int which, uint32_t i) -> int32_t& {
-    return i < (uint32_t)LISTCAP ? sm.uy[which][i] : reinterpret_cast<int32_t*>(spill_cta)[(which * 3 + 1) * CAP + (i - LISTCAP)];
-  };
-  auto list_c = [&](int which, uint32_t i) -> uint32_t& {
-    return i < (uint32_t)LISTCAP ? sm.uc[which][i] : spill_cta[(which * 3 + 2) * CAP + (i - LISTCAP)];
-  };
+  int32_t* const spill_i = reinterpret_cast<int32_t*>(spill_cta);
 
   if (tid == 0) {
     sm.li[0] = atomicAdd(&ctrl->work[CLS], 1u);
@@ -406,9 +414,12 @@ __global__ void __launch_bounds__(32 * W, MINB)
     for (uint32_t s = 0; s < S; ++s) {
       const uint32_t b0 = sm.off[3 * s], b1 = sm.off[3 * s + 1], b2 = sm.off[3 * s + 2], b3 = sm.off[3 * s + 3];
       const uint32_t n0 = b1 - b0, n1 = b2 - b1, n2 = b3 - b2;
-      const int32_t z0 = p.z[3 * s], z1 = p.z[3 * s + 1], z2 = p.z[3 * s + 2];
-      const int32_t M0 = p.key_mul[3 * s], M1 = p.key_mul[3 * s + 1], M2 = p.key_mul[3 * s + 2];
-      const int64_t T01 = p.thr_in[s][0], T02 = p.thr_in[s][1], T12 = p.thr_in[s][2];
+      StationConst c;
+      c.z0 = p.z[3 * s]; c.z1 = p.z[3 * s + 1]; c.z2 = p.z[3 * s + 2];
+      c.nz0 = -c.z0; c.nz1 = -c.z1; c.nz2 = -c.z2;
+      c.M0 = p.key_mul[3 * s]; c.M1 = p.key_mul[3 * s + 1]; c.M2 = p.key_mul[3 * s + 2];
+      c.T01 = p.thr_in[s][0]; c.T02 = p.thr_in[s][1]; c.T12 = p.thr_in[s][2];
+      c.T01x2 = p.thr2_in[s][0]; c.T02x2 = p.thr2_in[s][1]; c.T12x2 = p.thr2_in[s][2];
       if (tid == 0) { sm.acc = 0; sm.ucount = 0; }
       const bool search = (n0 != 0) & (n1 != 0) & (n2 != 0);
       if (search) {
@@ -423,11 +434,11 @@ __global__ void __launch_bounds__(32 * W, MINB)
           const bool l2 = i >= n0;
           const uint32_t g = l2 ? b2 + (i - n0) : b0 + i;
           const int32_t hx = __ldg(x + g), hy = __ldg(y + g);
-          const int32_t M = l2 ? M2 : M0;
-          const int c = (l2 ? ncell : 0) + bin_of(__mulhi(hx, M), kmin, sh, nb - 1) * nb +
-                        bin_of(__mulhi(hy, M), kmin, sh, nb - 1);
-          sm.cid[i] = (uint16_t)c;
-          atomicAdd(&cell[c], 1u);
+          const int32_t M = l2 ? c.M2 : c.M0;
+          const int cc = (l2 ? ncell : 0) + bin_of(__mulhi(hx, M), kmin, sh, nb - 1) * nb +
+                         bin_of(__mulhi(hy, M), kmin, sh, nb - 1);
+          sm.cid[i] = (uint16_t)cc;
+          atomicAdd(&cell[cc], 1u);
         }
         team_sync<W>();
         team_exclusive_scan<W>(cell, nvec, sm.wsum);
@@ -453,20 +464,16 @@ __global__ void __launch_bounds__(32 * W, MINB)
           if (act) {
             x1 = __ldg(x + b1 + i1);
             y1 = __ldg(y + b1 + i1);
-            r = rows_of(cell, 0, __mulhi(x1, M1), __mulhi(y1, M1), kmin, R, sh, nb);
+            r = rows_of(cell, 0, __mulhi(x1, c.M1), __mulhi(y1, c.M1), kmin, R, sh, nb);
           }
           const uint32_t nc = r.n0 + r.n1;
           const uint32_t ncmax = __reduce_max_sync(0xFFFFFFFFu, nc);
           // |x0*z1 - x1*z0| <= T01  <=>  (uint64)(x0*z1 + (T01 - x1*z0)) <= 2*T01
-          const int64_t Qx = T01 - (int64_t)x1 * z0, Qy = T01 - (int64_t)y1 * z0;
+          const int64_t Qx = anchor_q(x1, c.nz0, c.T01), Qy = anchor_q(y1, c.nz0, c.T01);
           for (uint32_t k = 0; k < ncmax; ++k) {
             const uint32_t j = k < r.n0 ? r.a0 + k : r.a1 + (k - r.n0);
             bool pass = false;
-            if (k < nc) {
-              const int32_t hx = sm.sx[j], hy = sm.sy[j];
-              pass = ((uint64_t)((int64_t)hx * z1 + Qx) <= 2 * (uint64_t)T01) &
-                     ((uint64_t)((int64_t)hy * z1 + Qy) <= 2 * (uint64_t)T01);
-            }
+            if (k < nc) pass = win_q(sm.sx[j], c.z1, Qx, c.T01x2) & win_q(sm.sy[j], c.z1, Qy, c.T01x2);
             const uint32_t pm = __ballot_sync(0xFFFFFFFFu, pass);
             if (pm) {
               if (pass) q[qn + __popc(pm & lanemask_lt())] = (j << 16) | i1;
@@ -476,9 +483,9 @@ __global__ void __launch_bounds__(32 * W, MINB)
                 qn -= 32;
                 const uint32_t ent = q[qn + lane];
                 const uint32_t j0 = ent >> 16, k1 = ent & 0xFFFFu;
-                const uint32_t c = count_h2(cell, sm.sx, sm.sy, ncell, sm.sx[j0], sm.sy[j0], __ldg(x + b1 + k1),
-                                            __ldg(y + b1 + k1), z0, z1, z2, T02, T12, M1, kmin, R, sh, nb);
-                if (c) atomicAdd(&sm.m[k1], c);
+                const uint32_t t = count_h2(sm, cell, ncell, c, sm.sx[j0], sm.sy[j0], __ldg(x + b1 + k1),
+                                            __ldg(y + b1 + k1), kmin, R, sh, nb);
+                if (t) atomicAdd(&sm.m[k1], t);
                 __syncwarp();
               }
             }
@@ -488,9 +495,9 @@ __global__ void __launch_bounds__(32 * W, MINB)
         if (lane < qn) {
           const uint32_t ent = q[lane];
           const uint32_t j0 = ent >> 16, k1 = ent & 0xFFFFu;
-          const uint32_t c = count_h2(cell, sm.sx, sm.sy, ncell, sm.sx[j0], sm.sy[j0], __ldg(x + b1 + k1),
-                                      __ldg(y + b1 + k1), z0, z1, z2, T02, T12, M1, kmin, R, sh, nb);
-          if (c) atomicAdd(&sm.m[k1], c);
+          const uint32_t t = count_h2(sm, cell, ncell, c, sm.sx[j0], sm.sy[j0], __ldg(x + b1 + k1), __ldg(y + b1 + k1),
+                                      kmin, R, sh, nb);
+          if (t) atomicAdd(&sm.m[k1], t);
         }
       }
       if (s == 0 && pf_b > pf_a) {  // pull the next event of this team into L2 while this one is being searched
@@ -504,40 +511,66 @@ __global__ void __launch_bounds__(32 * W, MINB)
 
       // ---- station total, list of distinct middle hits with triplets (R8)
       if (search) {
-        unsigned long long part = 0;
+        constexpr bool kSmallSum = (CAP + T - 1) / T < 8;  // 32 lanes * 7 hits * 2^24 < 2^32
+        uint32_t part32 = 0;
+        unsigned long long part64 = 0;
         for (uint32_t i = tid; i < n1; i += T) {
           const uint32_t mm = sm.m[i];
-          part += mm;
+          if (kSmallSum) part32 += mm; else part64 += mm;
           if (mm && !dead) {
             const uint32_t pos = atomicAdd(&sm.ucount, 1u);
-            list_x(cur, pos) = __ldg(x + b1 + i);
-            list_y(cur, pos) = __ldg(y + b1 + i);
-            list_c(cur, pos) = mm;
+            const int32_t hx = __ldg(x + b1 + i), hy = __ldg(y + b1 + i);
+            if (pos < (uint32_t)LISTCAP) {
+              sm.ux[cur][pos] = hx; sm.uy[cur][pos] = hy; sm.uc[cur][pos] = mm;
+            } else {
+              const uint32_t o = pos - LISTCAP;
+              spill_i[(cur * 3 + 0) * CAP + o] = hx; spill_i[(cur * 3 + 1) * CAP + o] = hy;
+              spill_cta[(cur * 3 + 2) * CAP + o] = mm;
+            }
           }
         }
+        if (kSmallSum) {
+          part32 = __reduce_add_sync(0xFFFFFFFFu, part32);
+          if (lane == 0 && part32) atomicAdd(&sm.acc, (unsigned long long)part32);
+        } else {
 #pragma unroll
-        for (int d = 16; d >= 1; d >>= 1) part += __shfl_xor_sync(0xFFFFFFFFu, part, d);
-        if (lane == 0 && part) atomicAdd(&sm.acc, part);
+          for (int d = 16; d >= 1; d >>= 1) part64 += __shfl_xor_sync(0xFFFFFFFFu, part64, d);
+          if (lane == 0 && part64) atomicAdd(&sm.acc, part64);
+        }
       }
       team_sync<W>();
       const uint32_t ncur = dead ? 0u : sm.ucount;
       if (tid == 0) n_triplets[(size_t)e * S + s] = sat32(sm.acc);
       // ---- a7: chain counts c_s[u] = m_u * sum over linked t of c_{s-1}[t], saturating (R9)
       if (s > 0 && !dead && ncur) {
-        const int32_t zA = p.z[3 * (s - 1) + 1], zB = z1;
+        const int32_t nzA = -p.z[3 * (s - 1) + 1], zB = c.z1;
         const int64_t TL = p.thr_link[s];
-        for (uint32_t u = tid; u < ncur; u += T) {
-          const int32_t xu = list_x(cur, u), yu = list_y(cur, u);
-          // |x_t*zB - x_u*zA| <= TL
-          const int64_t Qx = TL - (int64_t)xu * zA, Qy = TL - (int64_t)yu * zA;
-          unsigned long long a = 0;
-          for (uint32_t t = 0; t < nprev; ++t) {
-            const bool ok = ((uint64_t)((int64_t)list_x(cur ^ 1, t) * zB + Qx) <= 2 * (uint64_t)TL) &
-                            ((uint64_t)((int64_t)list_y(cur ^ 1, t) * zB + Qy) <= 2 * (uint64_t)TL);
-            if (ok) a += list_c(cur ^ 1, t);  // < 4096 * 2^32
+        const uint64_t TLx2 = p.thr2_link[s];
+        if (ncur <= (uint32_t)LISTCAP && nprev <= (uint32_t)LISTCAP) {  // everything in shared memory
+          for (uint32_t u = tid; u < ncur; u += T) {
+            // |x_t*zB - x_u*zA| <= TL
+            const int64_t Qx = anchor_q(sm.ux[cur][u], nzA, TL), Qy = anchor_q(sm.uy[cur][u], nzA, TL);
+            unsigned long long a = 0;
+            for (uint32_t t = 0; t < nprev; ++t) {
+              const bool ok = win_q(sm.ux[cur ^ 1][t], zB, Qx, TLx2) & win_q(sm.uy[cur ^ 1][t], zB, Qy, TLx2);
+              if (ok) a += sm.uc[cur ^ 1][t];  // < 4096 * 2^32
+            }
+            sm.uc[cur][u] = sat32((unsigned long long)sat32(a) * sm.uc[cur][u]);  // m_u <= 2^24: no overflow
           }
-          a = sat32(a);
-          list_c(cur, u) = sat32(a * (unsigned long long)list_c(cur, u));  // m_u <= 2^24: no overflow
+        } else {  // rare: some entries live in the global spill area
+          auto LX = [&](int w, uint32_t i) { return i < (uint32_t)LISTCAP ? sm.ux[w][i] : spill_i[(w * 3 + 0) * CAP + i - LISTCAP]; };
+          auto LY = [&](int w, uint32_t i) { return i < (uint32_t)LISTCAP ? sm.uy[w][i] : spill_i[(w * 3 + 1) * CAP + i - LISTCAP]; };
+          auto LC = [&](int w, uint32_t i) { return i < (uint32_t)LISTCAP ? sm.uc[w][i] : spill_cta[(w * 3 + 2) * CAP + i - LISTCAP]; };
+          for (uint32_t u = tid; u < ncur; u += T) {
+            const int64_t Qx = anchor_q(LX(cur, u), nzA, TL), Qy = anchor_q(LY(cur, u), nzA, TL);
+            unsigned long long a = 0;
+            for (uint32_t t = 0; t < nprev; ++t) {
+              const bool ok = win_q(LX(cur ^ 1, t), zB, Qx, TLx2) & win_q(LY(cur ^ 1, t), zB, Qy, TLx2);
+              if (ok) a += LC(cur ^ 1, t);
+            }
+            const uint32_t v = sat32((unsigned long long)sat32(a) * LC(cur, u));
+            if (u < (uint32_t)LISTCAP) sm.uc[cur][u] = v; else spill_cta[(cur * 3 + 2) * CAP + u - LISTCAP] = v;
+          }
         }
       }
       if (ncur == 0) dead = true;
@@ -551,16 +584,19 @@ __global__ void __launch_bounds__(32 * W, MINB)
     team_sync<W>();
     if (!dead) {
       unsigned long long part = 0;
-      for (uint32_t u = tid; u < nprev; u += T) part += list_c(cur ^ 1, u);
+      for (uint32_t u = tid; u < nprev; u += T)
+        part += u < (uint32_t)LISTCAP ? sm.uc[cur ^ 1][u] : spill_cta[((cur ^ 1) * 3 + 2) * CAP + u - LISTCAP];
+      if (__any_sync(0xFFFFFFFFu, part != 0)) {
 #pragma unroll
-      for (int d = 16; d >= 1; d >>= 1) part += __shfl_xor_sync(0xFFFFFFFFu, part, d);
-      if (lane == 0 && part) atomicAdd(&sm.acc, part);
+        for (int d = 16; d >= 1; d >>= 1) part += __shfl_xor_sync(0xFFFFFFFFu, part, d);
+        if (lane == 0) atomicAdd(&sm.acc, part);
+      }
     }
     team_sync<W>();
     if (tid == 0) {
-      const uint32_t c = sat32(sm.acc);
-      n_candidates[e] = c;
-      accept[e] = c >= p.min_candidates ? 1 : 0;
+      const uint32_t cand = sat32(sm.acc);
+      n_candidates[e] = cand;
+      accept[e] = cand >= p.min_candidates ? 1 : 0;
     }
     team_sync<W>();
   }

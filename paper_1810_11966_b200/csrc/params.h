@@ -23,6 +23,9 @@ struct Params {
   // window thresholds, R4: |x_h*z_B - x_g*z_A| <= T_AB = floor(a*z_A*z_B / b)  (left side is an integer)
   int64_t thr_in[kMaxStations][3];     // [s][0] = T01, [1] = T02, [2] = T12
   int64_t thr_link[kMaxStations];      // [s], s >= 1: middle layers of stations s-1 and s
+  // the same thresholds doubled: the test is evaluated as (uint64)(a*z_B + T - b*z_A) <= 2*T
+  uint64_t thr2_in[kMaxStations][3];
+  uint64_t thr2_link[kMaxStations];
   // slope keys used ONLY to choose which bins to look at (never to accept or reject a pair):
   // key(x, l) = mulhi(x, key_mul[l]) = floor(x * key_mul[l] / 2^32) ~ K * x / z_l, with |key - K*x/z_l| < 1.25
   int32_t key_mul[kMaxLayers];
