@@ -470,13 +470,26 @@ __global__ void __launch_bounds__(32 * W, MINB)
           const uint32_t ncmax = __reduce_max_sync(0xFFFFFFFFu, nc);
           // |x0*z1 - x1*z0| <= T01  <=>  (uint64)(x0*z1 + (T01 - x1*z0)) <= 2*T01
           const int64_t Qx = anchor_q(x1, c.nz0, c.T01), Qy = anchor_q(y1, c.nz0, c.T01);
-          for (uint32_t k = 0; k < ncmax; ++k) {
-            const uint32_t j = k < r.n0 ? r.a0 + k : r.a1 + (k - r.n0);
-            bool pass = false;
-            if (k < nc) pass = win_q(sm.sx[j], c.z1, Qx, c.T01x2) & win_q(sm.sy[j], c.z1, Qy, c.T01x2);
-            const uint32_t pm = __ballot_sync(0xFFFFFFFFu, pass);
-            if (pm) {
-              if (pass) q[qn + __popc(pm & lanemask_lt())] = (j << 16) | i1;
+          // test loop: no cross-lane traffic, each lane records its passing candidates as bits of `mask`
+          for (uint32_t k0 = 0; k0 < ncmax; k0 += 32) {
+            const uint32_t kend = min(ncmax - k0, 32u);
+            uint32_t mask = 0;
+            for (uint32_t kk = 0; kk < kend; ++kk) {
+              const uint32_t k = k0 + kk;
+              if (k < nc) {
+                const uint32_t j = k < r.n0 ? r.a0 + k : r.a1 + (k - r.n0);
+                const bool pass = win_q(sm.sx[j], c.z1, Qx, c.T01x2) & win_q(sm.sy[j], c.z1, Qy, c.T01x2);
+                mask |= (pass ? 1u : 0u) << kk;
+              }
+            }
+            // a6: rounds of ballot/popc compaction, one pair per lane and round, drained 32 at a time
+            for (uint32_t pm = __ballot_sync(0xFFFFFFFFu, mask != 0); pm; pm = __ballot_sync(0xFFFFFFFFu, mask != 0)) {
+              if (mask) {
+                const uint32_t k = k0 + (uint32_t)__ffs(mask) - 1u;
+                const uint32_t j = k < r.n0 ? r.a0 + k : r.a1 + (k - r.n0);
+                q[qn + __popc(pm & lanemask_lt())] = (j << 16) | i1;
+                mask &= mask - 1u;
+              }
               qn += __popc(pm);
               if (qn >= 32) {
                 __syncwarp();
