@@ -21,18 +21,18 @@ namespace {
 
 using namespace cbm;
 
-// team classes: warps per team, fullest layer admitted, uint4 vectors of bin counters (two grids of nb*nb),
+// team classes: warps per team, fullest layer admitted, coarse cells per axis the shared-memory tables hold,
 // middle hits per station kept in shared memory, resident CTAs per SM asked of the compiler
-constexpr int kMaxNbH = 40, kMaxNbM = 20;
-constexpr int kWM = 1, kCapM = 128, kNcvM = (2 * kMaxNbM * kMaxNbM + 3) / 4, kListM = 128, kMinBM = 16;
-constexpr int kWH = 4, kCapH = 448, kNcvH = (2 * kMaxNbH * kMaxNbH + 3) / 4, kListH = 64, kMinBH = 8;
-constexpr int kWG = 16, kCapG = 4096, kNcvG = kNcvH, kListG = 512, kMinBG = 1;
-using SmemM = TeamSmem<kWM, kCapM, kNcvM, kListM>;
-using SmemH = TeamSmem<kWH, kCapH, kNcvH, kListH>;
-using SmemG = TeamSmem<kWG, kCapG, kNcvG, kListG>;
-#define TEAM_KERNEL_M team_kernel<kWM, kCapM, kNcvM, kListM, kClsM, kMinBM, true>
-#define TEAM_KERNEL_H team_kernel<kWH, kCapH, kNcvH, kListH, kClsH, kMinBH, true>
-#define TEAM_KERNEL_G team_kernel<kWG, kCapG, kNcvG, kListG, kClsG, kMinBG, false>
+constexpr int kNfH = 64, kNfM = 32;  // fine cells per axis (at most); coarse = half
+constexpr int kWM = 1, kCapM = 128, kNcM = kNfM / 2, kListM = 128, kMinBM = 16;
+constexpr int kWH = 4, kCapH = 448, kNcH = kNfH / 2, kListH = 64, kMinBH = 8;
+constexpr int kWG = 16, kCapG = 4096, kNcG = kNfH / 2, kListG = 512, kMinBG = 1;
+using SmemM = TeamSmem<kWM, kCapM, kNcM, kListM>;
+using SmemH = TeamSmem<kWH, kCapH, kNcH, kListH>;
+using SmemG = TeamSmem<kWG, kCapG, kNcG, kListG>;
+#define TEAM_KERNEL_M team_kernel<kWM, kCapM, kNcM, kListM, kClsM, kMinBM, true>
+#define TEAM_KERNEL_H team_kernel<kWH, kCapH, kNcH, kListH, kClsH, kMinBH, true>
+#define TEAM_KERNEL_G team_kernel<kWG, kCapG, kNcG, kListG, kClsG, kMinBG, false>
 
 enum SlotState { kEmpty = 0, kUploaded = 1, kRunning = 2 };
 
@@ -154,50 +154,38 @@ int build_params(const cbm_trigger_config_t& c, Params& p, std::string& why) {
   p.tiny_max_total = tiny_on ? kTinyMaxTotal : 0;
   p.cls_max[kClsM] = kCapM; p.cls_max[kClsH] = kCapH; p.cls_max[kClsG] = kCapG;
 
-  // Slope keys (DESIGN.md "Binning is exact"): key = floor(x*M_l/2^32), M_l = round(2^32*K/z_l) < 2^31.
+  // Slope keys (DESIGN.md "The search is exact"): key = floor(x*M_l/2^32), M_l = round(2^32*K/z_l) < 2^31.
   // For any int32 x: |x*M_l/2^32 - K*x/z_l| <= 2^31 * 0.5/2^32 = 0.25, floor loses < 1  =>  |key - K*x/z_l| < 1.25.
   // Two hits with |x_h/z_A - x_g/z_B| <= w therefore have |key_h - key_g| < w*K + 2.5 <= R := ceil(w*K) + 3.
+  // Grid: nf fine cells of 2^fsh keys per axis cover the slope range (outliers share the edge cells); a fine
+  // cell must be at least R wide (compatible hits lie in fine cells at most one apart; a coarse cell = two fine
+  // cells >= 2R, so a window touches at most 2 x 2 coarse cells).  Largest nf first, then the largest K.
   const double w = (double)c.win_in_num / (double)c.win_in_den;
   const double smax = (c.slope_range_milli ? c.slope_range_milli : 400) / 1000.0;
   const double Kmax = 0.499 * (double)p.z[0];
-  double cell = std::max(2.0 * w * 1.05, 2.0 * smax / 44.0);
+  int nf = 1, fsh = 30, R = 0;
+  double K = Kmax;
   bool ok = false;
-  int sh = 0;
-  double K = 0;
-  int R = 0;
-  for (int it = 0; it < 64 && !ok; ++it, cell *= 1.25) {
-    const double lim = cell * Kmax;
-    if (lim < 4.0) break;
-    sh = (int)std::floor(std::log2(lim));
-    if (sh > 14) sh = 14;
-    K = std::ldexp(1.0, sh) / cell;
-    R = (int)std::ceil(w * K) + 3;
-    ok = 2 * R <= (1 << sh);
+  for (int n = kNfH; n >= 2 && !ok; n >>= 1) {
+    for (int sh = 14; sh >= 2 && !ok; --sh) {
+      const double k = ((double)n * std::ldexp(1.0, sh) - 2.0) / (2.0 * smax);  // n * 2^sh keys span the range
+      if (k > Kmax || k < 4.0) continue;
+      const int r = (int)std::ceil(w * k) + 3;
+      if (r <= (1 << sh)) { ok = true; nf = n; fsh = sh; K = k; R = r; }
+    }
   }
-  if (!ok) {  // geometry too fine for the key resolution: one bin per layer (still exact, just slower)
-    K = Kmax; sh = 30; R = 0;
-    for (int c3 = 0; c3 < kNumTeamClasses; ++c3) { p.cls_shift[c3] = 30; p.cls_nb[c3] = 1; }
-    p.key_min = 0;
-  } else {
-    const int half = (int)std::ceil(smax * K);
-    p.key_min = -half;
-    int shH = sh;
-    while (((2 * half) >> shH) + 1 > kMaxNbH) ++shH;
-    p.cls_shift[kClsH] = p.cls_shift[kClsG] = shH;
-    p.cls_nb[kClsH] = p.cls_nb[kClsG] = (uint32_t)(((2 * half) >> shH) + 1);
-    p.cls_shift[kClsM] = shH + 1;
-    p.cls_nb[kClsM] = (uint32_t)(((2 * half) >> (shH + 1)) + 1);
-  }
+  // !ok: geometry too fine for the key resolution: one cell per layer (still exact, just slower)
   p.key_R = R;
+  p.key_min = ok ? -(int)std::ceil(smax * K) : 0;
+  p.cls_nf[kClsH] = p.cls_nf[kClsG] = (uint32_t)nf;
+  p.cls_fsh[kClsH] = p.cls_fsh[kClsG] = fsh;
+  if (nf >= 2) { p.cls_nf[kClsM] = (uint32_t)std::min(nf / 2, kNfM); p.cls_fsh[kClsM] = fsh + (nf / 2 <= kNfM ? 1 : 2); }
+  else { p.cls_nf[kClsM] = 1; p.cls_fsh[kClsM] = fsh; }
   for (uint32_t l = 0; l < p.L; ++l) {
     const double m = std::ldexp(K, 32) / (double)p.z[l];
     const long long mi = llround(m);
     if (mi < 0 || mi > 0x7FFFFFFFll) { why = "internal: key multiplier out of range"; return CBM_ERR_INVALID_ARG; }
     p.key_mul[l] = (int32_t)mi;
-  }
-  if (p.cls_nb[kClsM] > (uint32_t)kMaxNbM || p.cls_nb[kClsH] > (uint32_t)kMaxNbH) {
-    why = "internal: bin grid too large";
-    return CBM_ERR_INVALID_ARG;
   }
   return CBM_OK;
 }

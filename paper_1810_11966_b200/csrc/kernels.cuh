@@ -244,64 +244,45 @@ __global__ void __launch_bounds__(kTileEvents* kMaxStations)
 // ================================================================================================ team kernel
 // One team = one CTA of W warps works on one event at a time (persistent: events are fetched from the class
 // list with an atomic cursor, two fetches ahead so that the next event can be prefetched into L2).
-// CAP = fullest layer the class admits; NCV = uint4 vectors of bin counters (both binned layers of a station);
+// CAP = fullest layer the class admits; NC = coarse cells per axis the shared-memory tables are sized for;
 // LISTCAP = middle hits with triplets kept in shared memory per station (more spill to a global scratch).
+//
+// Per station:
+//   stage   one 1-D TMA bulk copy per coordinate brings the station's three layers (contiguous in x[], y[])
+//           into shared memory; it is issued as soon as the previous station's search is over, so its flight
+//           overlaps the previous station's linking.
+//   A       every hit of layers 0 and 2 is pushed on the chain of its coarse slope cell (atomicExch on the
+//           cell's head, `next` link per hit) and sets its bit in the layer's fine occupancy bitmap
+//           (fine cell = half a coarse cell >= key_R).
+//   B       J = dilate3x3(occ0) & dilate3x3(occ2), by row-wise shifts and ORs of 64-bit rows.
+//   C       a middle hit h1 whose fine cell is not in J cannot have both a compatible h0 and a compatible h2
+//           (proof: DESIGN.md "The search is exact"); the others are compacted (ballot/popc) into a list.
+//   D       one lane per surviving h1: walks the chains of the <= 2x2 coarse cells around it in layer 0
+//           (exact test), then in layer 2 (exact tests against h1 and against the recorded h0), and appends
+//           (x1, y1, number of triplets with this middle hit) to the station's list  (R8).
+//   F       chain counts against the previous station's list (a7), result write (a8).
 template <int W>
 __device__ __forceinline__ void team_sync() {
   if (W == 1) __syncwarp(); else __syncthreads();
 }
 
-template <int W, int CAP, int NCV, int LISTCAP>
+template <int W, int CAP, int NC, int LISTCAP>
 struct TeamSmem {
-  alignas(16) uint32_t cellraw[4 + 4 * NCV];  // cell = cellraw + 4: cell[k] = end of bin k after the scatter, cell[-1] = 0
-  int32_t sx[2 * CAP], sy[2 * CAP];           // layer 0 then layer 2 of the station, bin-sorted
-  uint32_t m[CAP];                            // m[i1] = number of triplets with middle hit i1   (R8)
-  int32_t ux[2][LISTCAP], uy[2][LISTCAP];     // distinct middle hits with m > 0 of the previous / current station
-  uint32_t uc[2][LISTCAP];                    // their saturated chain counts c_s[u]
-  uint32_t queue[W][64];                      // per-warp queue of compatible (h0,h1) pairs: (j_sorted << 16) | i1
-  uint16_t cid[2 * CAP];                      // bin of every hit of layers 0 and 2 (count pass -> scatter pass)
+  alignas(16) int32_t sx[3 * CAP + 8];        // the station as it lies in x[] (from the 16-byte boundary below its
+  alignas(16) int32_t sy[3 * CAP + 8];        // first hit): layer 0, layer 1, layer 2
+  alignas(16) uint32_t head[2 * NC * NC];     // chain heads (hit index in its layer + 1; 0 = empty) of layers 0 and 2
+  uint32_t occ[2][128];                       // fine occupancy bitmaps of layers 0 and 2: row fx = 2 words, bit fy
+  uint32_t J[128];                            // dilate(occ[0]) & dilate(occ[1])
+  uint16_t next[2][CAP];                      // chain links (index + 1; 0 = end)
+  uint16_t surv[CAP];                         // middle hits that passed the bitmap filter
+  int32_t ux[2][LISTCAP], uy[2][LISTCAP];     // middle hits with triplets of the previous / current station
+  uint32_t uc[2][LISTCAP];                    // their multiplicities, then saturated chain counts c_s[u]
   uint32_t off[kMaxLayers + 1];
-  uint32_t wsum[32];
-  unsigned long long acc;                     // block-wide u64 accumulator (triplet total / candidate total)
-  uint32_t ucount;
+  unsigned long long acc[2];                  // triplets of the station (parity-buffered with the two below)
+  uint32_t nsurv[2], ucount[2];
   uint32_t li[3];                             // ring of fetched work indices
+  alignas(8) uint64_t bar;                    // completion of the station's bulk copies
 };
-
-// in-place exclusive scan of cell[0 .. 4*nvec) by the whole team, 128-bit shared-memory accesses
-template <int W>
-__device__ __forceinline__ void team_exclusive_scan(uint32_t* cell, uint32_t nvec, uint32_t* wsum) {
-  constexpr uint32_t T = 32 * W;
-  const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const uint32_t chunk = (nvec + T - 1) / T;
-  const uint32_t lo = min(tid * chunk, nvec), hi = min(lo + chunk, nvec);
-  uint4* const v = reinterpret_cast<uint4*>(cell);
-  uint32_t sum = 0;
-  for (uint32_t i = lo; i < hi; ++i) {
-    const uint4 c = v[i];
-    sum += c.x + c.y + c.z + c.w;
-  }
-  uint32_t incl = sum;
-#pragma unroll
-  for (int d = 1; d < 32; d <<= 1) {
-    const uint32_t u = __shfl_up_sync(0xFFFFFFFFu, incl, d);
-    if (lane >= (uint32_t)d) incl += u;
-  }
-  uint32_t base = incl - sum;
-  if (W > 1) {
-    if (lane == 31) wsum[warp] = incl;
-    __syncthreads();
-    uint32_t wv = (lane < (uint32_t)W && lane < warp) ? wsum[lane] : 0u;
-    wv = __reduce_add_sync(0xFFFFFFFFu, wv);
-    base += wv;
-  }
-  for (uint32_t i = lo; i < hi; ++i) {
-    const uint4 c = v[i];
-    uint4 o;
-    o.x = base; o.y = o.x + c.x; o.z = o.y + c.y; o.w = o.z + c.z;
-    base = o.w + c.w;
-    v[i] = o;
-  }
-}
 
 __device__ __forceinline__ int bin_of(int key, int kmin, int sh, int nbm1) {
   return min(max((key - kmin) >> sh, 0), nbm1);
@@ -315,82 +296,104 @@ __device__ __forceinline__ bool win_q(int32_t a, int32_t zo, int64_t Q, uint64_t
   return (uint64_t)((int64_t)a * zo + Q) <= T2;
 }
 
-// The bins that can hold a hit compatible with a hit of slope keys (kx, ky): at most two rows (bx) of
-// consecutive bins, because 2*R <= 2^shift.  Rows as index ranges [a0, a0+n0), [a1, a1+n1) of the bin-sorted
-// layer whose bins start at cell[base].
-struct Rows { uint32_t a0, n0, a1, n1; };
-__device__ __forceinline__ Rows rows_of(const uint32_t* cell, int base, int kx, int ky, int kmin, int R, int sh, int nb) {
-  const int tx = kx - R - kmin, ty = ky - R - kmin;
-  const int bxl = min(max(tx >> sh, 0), nb - 1), bxh = min(max((tx + 2 * R) >> sh, 0), nb - 1);
-  const int byl = min(max(ty >> sh, 0), nb - 1), byh = min(max((ty + 2 * R) >> sh, 0), nb - 1);
-  const int r0 = base + bxl * nb, r1 = base + bxh * nb;
-  Rows r;
-  r.a0 = cell[r0 + byl - 1];
-  r.n0 = cell[r0 + byh] - r.a0;
-  r.a1 = cell[r1 + byl - 1];
-  r.n1 = bxh != bxl ? cell[r1 + byh] - r.a1 : 0u;
-  return r;
-}
-
 // per-station constants, loaded once per station
 struct StationConst {
-  int32_t z0, z1, z2, nz0, nz1, nz2;  // nz = -z
+  int32_t z0, z1, z2, nz0, nz2;  // nz = -z
   int32_t M0, M1, M2;
   int64_t T01, T02, T12;
   uint64_t T01x2, T02x2, T12x2;
 };
 
-// Phase 2 (a5): for one compatible (h0,h1) pair, count the h2 of layer 2 compatible with both.
-// Looks only at the 2-D bins around h1's slope (superset of its window), tests exactly.
-template <class SM>
-__device__ __forceinline__ uint32_t count_h2(const SM& sm, const uint32_t* cell, int ncell, const StationConst& c,
-                                             int32_t x0, int32_t y0, int32_t x1, int32_t y1, int kmin, int R, int sh,
-                                             int nb) {
-  const Rows r = rows_of(cell, ncell, __mulhi(x1, c.M1), __mulhi(y1, c.M1), kmin, R, sh, nb);
-  const uint32_t n = r.n0 + r.n1;
-  if (n == 0) return 0;
-  // |x2*z1 - x1*z2| <= T12 and |x2*z0 - x0*z2| <= T02 (and the same in y)
-  const int64_t Qx1 = anchor_q(x1, c.nz2, c.T12), Qy1 = anchor_q(y1, c.nz2, c.T12);
-  const int64_t Qx0 = anchor_q(x0, c.nz2, c.T02), Qy0 = anchor_q(y0, c.nz2, c.T02);
-  uint32_t cnt = 0;
-  for (uint32_t k = 0; k < n; ++k) {
-    const uint32_t j = k < r.n0 ? r.a0 + k : r.a1 + (k - r.n0);
-    const int32_t x2 = sm.sx[j], y2 = sm.sy[j];
-    const bool ok = win_q(x2, c.z1, Qx1, c.T12x2) & win_q(y2, c.z1, Qy1, c.T12x2) & win_q(x2, c.z0, Qx0, c.T02x2) &
-                    win_q(y2, c.z0, Qy0, c.T02x2);
-    cnt += ok ? 1u : 0u;
-  }
-  return cnt;
+// Chain heads of the <= 2x2 coarse cells that can hold a hit compatible with a hit whose window starts in
+// `cell` (dx / dy: the window reaches the next cell row / column); non-empty heads first.
+struct Heads { uint32_t a, b, c, d; };
+__device__ __forceinline__ Heads load_heads(const uint32_t* head, uint32_t cell, bool dx, bool dy, int nc) {
+  Heads h;
+  h.a = head[cell];
+  h.b = dy ? head[cell + 1] : 0u;
+  h.c = dx ? head[cell + nc] : 0u;
+  h.d = (dx && dy) ? head[cell + nc + 1] : 0u;
+  if (!h.c) { h.c = h.d; h.d = 0; }
+  if (!h.b) { h.b = h.c; h.c = h.d; h.d = 0; }
+  if (!h.a) { h.a = h.b; h.b = h.c; h.c = h.d; h.d = 0; }
+  return h;
 }
 
-template <int W, int CAP, int NCV, int LISTCAP, int CLS, int MINB, bool STATIC_SMEM>
+// Rare path of phase D (a middle hit with more than three compatible h0): number of h0 in the <= 2x2 cells
+// compatible with both h1 (anchors Qx, Qy) and h2 (x2, y2).  No warp-level operation inside.
+template <class SM>
+__device__ __noinline__ uint32_t count_h0_slow(const SM& sm, const uint32_t* head, uint32_t o0, uint32_t cell, bool dx,
+                                               bool dy, int nc, const StationConst& c, int64_t Qx, int64_t Qy, int32_t x2,
+                                               int32_t y2) {
+  uint32_t n = 0;
+  for (int q = 0; q < 4; ++q) {
+    if ((q & 1) && !dy) continue;
+    if ((q & 2) && !dx) continue;
+    for (uint32_t cur = head[cell + (q & 1) + ((q & 2) ? nc : 0)]; cur; cur = sm.next[0][cur - 1]) {
+      const int32_t x0 = sm.sx[o0 + cur - 1], y0 = sm.sy[o0 + cur - 1];
+      const bool ok = win_q(x0, c.z1, Qx, c.T01x2) & win_q(y0, c.z1, Qy, c.T01x2) &
+                      win_q(x2, c.z0, anchor_q(x0, c.nz2, c.T02), c.T02x2) &
+                      win_q(y2, c.z0, anchor_q(y0, c.nz2, c.T02), c.T02x2);
+      n += ok ? 1u : 0u;
+    }
+  }
+  return n;
+}
+
+template <int W, int CAP, int NC, int LISTCAP, int CLS, int MINB, bool STATIC_SMEM>
 __global__ void __launch_bounds__(32 * W, MINB)
     team_kernel(const __grid_constant__ Params p, const int32_t* __restrict__ x, const int32_t* __restrict__ y,
                 const uint32_t* __restrict__ off, uint32_t* __restrict__ n_triplets, uint32_t* __restrict__ n_candidates,
                 uint8_t* __restrict__ accept, Ctrl* __restrict__ ctrl, const uint32_t* __restrict__ list,
                 uint32_t* __restrict__ spill) {
-  using SM = TeamSmem<W, CAP, NCV, LISTCAP>;
+  using SM = TeamSmem<W, CAP, NC, LISTCAP>;
   extern __shared__ __align__(16) unsigned char smem_dyn[];
   __shared__ __align__(16) unsigned char smem_static[STATIC_SMEM ? sizeof(SM) : 16];
   SM& sm = *reinterpret_cast<SM*>(STATIC_SMEM ? smem_static : smem_dyn);
   constexpr uint32_t T = 32 * W;
+  constexpr uint32_t FULL = 0xFFFFFFFFu;
+  constexpr uint32_t kZeroVec = (2 * NC * NC + 256) / 4;  // head[] and occ[][] are contiguous
+  static_assert((2 * NC * NC) % 4 == 0 && offsetof(SM, occ) == offsetof(SM, head) + 2 * NC * NC * 4, "layout");
   const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const uint32_t S = p.S, L = p.L;
   const uint32_t n_list = ctrl->count[CLS];
-  const int kmin = p.key_min, R = p.key_R, sh = p.cls_shift[CLS], nb = (int)p.cls_nb[CLS];
-  const int ncell = nb * nb;
-  const uint32_t nvec = (uint32_t)(2 * ncell + 3) >> 2;
-  uint32_t* const cell = sm.cellraw + 4;
+  const int kmin = p.key_min, R = p.key_R, fsh = p.cls_fsh[CLS], csh = fsh + 1;
+  const int nf1 = (int)p.cls_nf[CLS] - 1;
+  const int nc = max((int)p.cls_nf[CLS] >> 1, 1), nc1 = nc - 1;
+  uint32_t* const head0 = sm.head;
+  uint32_t* const head2 = sm.head + nc * nc;
   // spill area of this CTA: list entries beyond LISTCAP, [2 lists][x, y, c][CAP] words
   uint32_t* const spill_cta = spill + (size_t)blockIdx.x * 6 * CAP;
   int32_t* const spill_i = reinterpret_cast<int32_t*>(spill_cta);
 
+  {
+    uint4* const v = reinterpret_cast<uint4*>(sm.head);
+    for (uint32_t i = tid; i < kZeroVec; i += T) v[i] = make_uint4(0, 0, 0, 0);
+  }
   if (tid == 0) {
     sm.li[0] = atomicAdd(&ctrl->work[CLS], 1u);
     sm.li[1] = atomicAdd(&ctrl->work[CLS], 1u);
-    sm.cellraw[3] = 0;
+    sm.acc[0] = sm.acc[1] = 0;
+    sm.nsurv[0] = sm.nsurv[1] = 0;
+    sm.ucount[0] = sm.ucount[1] = 0;
+    mbar_init(&sm.bar, 1);
+    fence_mbar_init();
   }
   team_sync<W>();
+  uint32_t par = 0;  // phase parity of the staging barrier
+  uint32_t sp = 0;   // parity of the per-station counters
+
+  // a4: thread 0 starts the bulk copies of station s of the event whose offsets are in sm.off
+  auto searchable = [&](uint32_t s) {
+    return (sm.off[3 * s] != sm.off[3 * s + 1]) & (sm.off[3 * s + 1] != sm.off[3 * s + 2]) & (sm.off[3 * s + 2] != sm.off[3 * s + 3]);
+  };
+  auto issue_stage = [&](uint32_t s) {
+    const uint32_t a = sm.off[3 * s] & ~3u;
+    const uint32_t bytes = (((sm.off[3 * s + 3] + 3u) & ~3u) - a) * 4u;  // <= (3*CAP + 6) * 4
+    mbar_arrive_expect_tx(&sm.bar, 2u * bytes);
+    bulk_g2s(sm.sx, x + a, bytes, &sm.bar);
+    bulk_g2s(sm.sy, y + a, bytes, &sm.bar);
+  };
 
   for (uint32_t it3 = 0;; it3 = it3 == 2 ? 0 : it3 + 1) {
     const uint32_t li = sm.li[it3];
@@ -398,7 +401,7 @@ __global__ void __launch_bounds__(32 * W, MINB)
     const uint32_t nxt = sm.li[it3 == 2 ? 0 : it3 + 1];
     if (tid == 0) sm.li[it3 == 0 ? 2 : it3 - 1] = atomicAdd(&ctrl->work[CLS], 1u);
     const uint32_t e = __ldg(list + li);
-    // extent of the NEXT event: loaded now, used for its L2 prefetch after station 0 (latency hidden)
+    // extent of the NEXT event: loaded now, used for its L2 prefetch during station 0 (latency hidden)
     uint32_t pf_a = 0, pf_b = 0;
     if (nxt < n_list) {
       const uint32_t e2 = __ldg(list + nxt);
@@ -407,6 +410,7 @@ __global__ void __launch_bounds__(32 * W, MINB)
     }
     for (uint32_t i = tid; i <= L; i += T) sm.off[i] = __ldg(off + (size_t)e * L + i);
     team_sync<W>();
+    if (tid == 0 && searchable(0)) issue_stage(0);
 
     uint32_t nprev = 0;
     bool dead = false;  // some station so far has no triplet => no chain; triplet counts are still needed
@@ -414,104 +418,174 @@ __global__ void __launch_bounds__(32 * W, MINB)
     for (uint32_t s = 0; s < S; ++s) {
       const uint32_t b0 = sm.off[3 * s], b1 = sm.off[3 * s + 1], b2 = sm.off[3 * s + 2], b3 = sm.off[3 * s + 3];
       const uint32_t n0 = b1 - b0, n1 = b2 - b1, n2 = b3 - b2;
+      const uint32_t o0 = b0 & 3u, o1 = o0 + n0, o2 = o1 + n1;  // layer starts in sm.sx / sm.sy
       StationConst c;
       c.z0 = p.z[3 * s]; c.z1 = p.z[3 * s + 1]; c.z2 = p.z[3 * s + 2];
-      c.nz0 = -c.z0; c.nz1 = -c.z1; c.nz2 = -c.z2;
+      c.nz0 = -c.z0; c.nz2 = -c.z2;
       c.M0 = p.key_mul[3 * s]; c.M1 = p.key_mul[3 * s + 1]; c.M2 = p.key_mul[3 * s + 2];
       c.T01 = p.thr_in[s][0]; c.T02 = p.thr_in[s][1]; c.T12 = p.thr_in[s][2];
       c.T01x2 = p.thr2_in[s][0]; c.T02x2 = p.thr2_in[s][1]; c.T12x2 = p.thr2_in[s][2];
-      if (tid == 0) { sm.acc = 0; sm.ucount = 0; }
       const bool search = (n0 != 0) & (n1 != 0) & (n2 != 0);
       if (search) {
-        // ---- a4: bin layers 0 and 2 on a 2-D slope grid: count, one scan over both grids, scatter
-        {
-          uint4* const v = reinterpret_cast<uint4*>(cell);
-          for (uint32_t i = tid; i < nvec; i += T) v[i] = make_uint4(0, 0, 0, 0);
-          for (uint32_t i = tid; i < n1; i += T) sm.m[i] = 0;
+        while (!mbar_try_wait(&sm.bar, par)) {
         }
-        team_sync<W>();
+        par ^= 1u;
+        // ---- A: chains of layers 0 and 2 on the coarse grid, fine occupancy bitmaps
         for (uint32_t i = tid; i < n0 + n2; i += T) {
           const bool l2 = i >= n0;
-          const uint32_t g = l2 ? b2 + (i - n0) : b0 + i;
-          const int32_t hx = __ldg(x + g), hy = __ldg(y + g);
+          const uint32_t j = l2 ? i - n0 : i;
+          const uint32_t si = (l2 ? o2 : o0) + j;
           const int32_t M = l2 ? c.M2 : c.M0;
-          const int cc = (l2 ? ncell : 0) + bin_of(__mulhi(hx, M), kmin, sh, nb - 1) * nb +
-                         bin_of(__mulhi(hy, M), kmin, sh, nb - 1);
-          sm.cid[i] = (uint16_t)cc;
-          atomicAdd(&cell[cc], 1u);
+          const int fx = bin_of(__mulhi(sm.sx[si], M), kmin, fsh, nf1), fy = bin_of(__mulhi(sm.sy[si], M), kmin, fsh, nf1);
+          uint32_t* const hd = l2 ? head2 : head0;
+          const uint32_t old = atomicExch(&hd[(fx >> 1) * nc + (fy >> 1)], j + 1u);
+          sm.next[l2 ? 1 : 0][j] = (uint16_t)old;
+          atomicOr(&sm.occ[l2 ? 1 : 0][2 * fx + (fy >> 5)], 1u << (fy & 31));
         }
         team_sync<W>();
-        team_exclusive_scan<W>(cell, nvec, sm.wsum);
-        team_sync<W>();
-        for (uint32_t i = tid; i < n0 + n2; i += T) {
-          const uint32_t g = i >= n0 ? b2 + (i - n0) : b0 + i;
-          const int32_t hx = __ldg(x + g), hy = __ldg(y + g);  // L1 hit
-          const uint32_t pos = atomicAdd(&cell[sm.cid[i]], 1u);
-          sm.sx[pos] = hx;
-          sm.sy[pos] = hy;
+        // ---- B: J = dilate(occ0) & dilate(occ2); a compatible pair lies in fine cells at most one apart
+        for (uint32_t r = tid; r < 64; r += T) {
+          unsigned long long d[2];
+#pragma unroll
+          for (int l = 0; l < 2; ++l) {
+            const unsigned long long* rows = reinterpret_cast<const unsigned long long*>(sm.occ[l]);
+            unsigned long long v = rows[r];
+            if (r > 0) v |= rows[r - 1];
+            if (r < 63) v |= rows[r + 1];
+            d[l] = v | (v << 1) | (v >> 1);
+          }
+          const unsigned long long j = d[0] & d[1];
+          sm.J[2 * r] = (uint32_t)j;
+          sm.J[2 * r + 1] = (uint32_t)(j >> 32);
         }
         team_sync<W>();
-
-        // ---- a5/a6: anchors = middle-layer hits, one per lane; compatible (h0,h1) pairs are compacted
-        // into the warp's queue with ballot/popc and drained 32 at a time by phase 2.
-        uint32_t qn = 0;
-        uint32_t* const q = sm.queue[warp];
+        // ---- C (a6): middle hits whose fine cell is in J, compacted with ballot/popc
         for (uint32_t base = warp * 32; base < n1; base += T) {
           const uint32_t i1 = base + lane;
-          const bool act = i1 < n1;
+          bool keep = false;
+          if (i1 < n1) {
+            const int fx = bin_of(__mulhi(sm.sx[o1 + i1], c.M1), kmin, fsh, nf1);
+            const int fy = bin_of(__mulhi(sm.sy[o1 + i1], c.M1), kmin, fsh, nf1);
+            keep = (sm.J[2 * fx + (fy >> 5)] >> (fy & 31)) & 1u;
+          }
+          const uint32_t km = __ballot_sync(FULL, keep);
+          if (km) {
+            const int leader = __ffs(km) - 1;
+            uint32_t pos = 0;
+            if ((int)lane == leader) pos = atomicAdd(&sm.nsurv[sp], (uint32_t)__popc(km));
+            pos = __shfl_sync(FULL, pos, leader);
+            if (keep) sm.surv[pos + __popc(km & lanemask_lt())] = (uint16_t)i1;
+          }
+        }
+        team_sync<W>();
+        // ---- D (a5): one lane per surviving middle hit
+        const uint32_t nsv = sm.nsurv[sp];
+        unsigned long long trip = 0;
+        for (uint32_t cb = warp * 32; cb < nsv; cb += T) {
+          const bool act = cb + lane < nsv;
           int32_t x1 = 0, y1 = 0;
-          Rows r = {0, 0, 0, 0};
+          uint32_t cell = 0;
+          bool dx = false, dy = false;
+          Heads h = {0, 0, 0, 0};
           if (act) {
-            x1 = __ldg(x + b1 + i1);
-            y1 = __ldg(y + b1 + i1);
-            r = rows_of(cell, 0, __mulhi(x1, c.M1), __mulhi(y1, c.M1), kmin, R, sh, nb);
+            const uint32_t i1 = sm.surv[cb + lane];
+            x1 = sm.sx[o1 + i1];
+            y1 = sm.sy[o1 + i1];
+            const int tx = __mulhi(x1, c.M1) - R - kmin, ty = __mulhi(y1, c.M1) - R - kmin;
+            const int lox = min(max(tx >> csh, 0), nc1), hix = min(max((tx + 2 * R) >> csh, 0), nc1);
+            const int loy = min(max(ty >> csh, 0), nc1), hiy = min(max((ty + 2 * R) >> csh, 0), nc1);
+            cell = (uint32_t)(lox * nc + loy);
+            dx = hix != lox;
+            dy = hiy != loy;
+            h = load_heads(head0, cell, dx, dy, nc);
           }
-          const uint32_t nc = r.n0 + r.n1;
-          const uint32_t ncmax = __reduce_max_sync(0xFFFFFFFFu, nc);
-          // |x0*z1 - x1*z0| <= T01  <=>  (uint64)(x0*z1 + (T01 - x1*z0)) <= 2*T01
+          // h0 compatible with h1:  |x0*z1 - x1*z0| <= T01  <=>  (uint64)(x0*z1 + (T01 - x1*z0)) <= 2*T01
           const int64_t Qx = anchor_q(x1, c.nz0, c.T01), Qy = anchor_q(y1, c.nz0, c.T01);
-          // test loop: no cross-lane traffic, each lane records its passing candidates as bits of `mask`
-          for (uint32_t k0 = 0; k0 < ncmax; k0 += 32) {
-            const uint32_t kend = min(ncmax - k0, 32u);
-            uint32_t mask = 0;
-            for (uint32_t kk = 0; kk < kend; ++kk) {
-              const uint32_t k = k0 + kk;
-              if (k < nc) {
-                const uint32_t j = k < r.n0 ? r.a0 + k : r.a1 + (k - r.n0);
-                const bool pass = win_q(sm.sx[j], c.z1, Qx, c.T01x2) & win_q(sm.sy[j], c.z1, Qy, c.T01x2);
-                mask |= (pass ? 1u : 0u) << kk;
+          uint32_t np = 0, p0 = 0, p1 = 0, p2 = 0;  // number of compatible h0, the first three (index + 1)
+          uint32_t cu = h.a;
+          while (__any_sync(FULL, cu != 0)) {
+            if (cu) {
+              const uint32_t j = cu - 1u;
+              const int32_t x0 = sm.sx[o0 + j], y0 = sm.sy[o0 + j];
+              const uint32_t nx = sm.next[0][j];
+              if (win_q(x0, c.z1, Qx, c.T01x2) & win_q(y0, c.z1, Qy, c.T01x2)) {
+                if (np == 0) p0 = cu; else if (np == 1) p1 = cu; else if (np == 2) p2 = cu;
+                ++np;
+              }
+              cu = nx;
+              if (!cu) { cu = h.b; h.b = h.c; h.c = h.d; h.d = 0; }
+            }
+          }
+          uint32_t t = 0;  // triplets with this middle hit
+          if (__any_sync(FULL, np != 0)) {
+            Heads g = {0, 0, 0, 0};
+            if (np) g = load_heads(head2, cell, dx, dy, nc);
+            // h2 compatible with h1:  |x2*z1 - x1*z2| <= T12;  with h0:  |x2*z0 - x0*z2| <= T02
+            const int64_t Rx = anchor_q(x1, c.nz2, c.T12), Ry = anchor_q(y1, c.nz2, c.T12);
+            cu = g.a;
+            while (__any_sync(FULL, cu != 0)) {
+              if (cu) {
+                const uint32_t j = cu - 1u;
+                const int32_t x2 = sm.sx[o2 + j], y2 = sm.sy[o2 + j];
+                const uint32_t nx = sm.next[1][j];
+                if (win_q(x2, c.z1, Rx, c.T12x2) & win_q(y2, c.z1, Ry, c.T12x2)) {
+                  if (np <= 3) {
+                    uint32_t pk = p0;
+                    for (uint32_t k = 0; k < np; ++k) {
+                      const int32_t x0 = sm.sx[o0 + pk - 1u], y0 = sm.sy[o0 + pk - 1u];
+                      const bool ok = win_q(x2, c.z0, anchor_q(x0, c.nz2, c.T02), c.T02x2) &
+                                      win_q(y2, c.z0, anchor_q(y0, c.nz2, c.T02), c.T02x2);
+                      t += ok ? 1u : 0u;
+                      pk = k == 0 ? p1 : p2;
+                    }
+                  } else {
+                    t += count_h0_slow(sm, head0, o0, cell, dx, dy, nc, c, Qx, Qy, x2, y2);
+                  }
+                }
+                cu = nx;
+                if (!cu) { cu = g.b; g.b = g.c; g.c = g.d; g.d = 0; }
               }
             }
-            // a6: rounds of ballot/popc compaction, one pair per lane and round, drained 32 at a time
-            for (uint32_t pm = __ballot_sync(0xFFFFFFFFu, mask != 0); pm; pm = __ballot_sync(0xFFFFFFFFu, mask != 0)) {
-              if (mask) {
-                const uint32_t k = k0 + (uint32_t)__ffs(mask) - 1u;
-                const uint32_t j = k < r.n0 ? r.a0 + k : r.a1 + (k - r.n0);
-                q[qn + __popc(pm & lanemask_lt())] = (j << 16) | i1;
-                mask &= mask - 1u;
-              }
-              qn += __popc(pm);
-              if (qn >= 32) {
-                __syncwarp();
-                qn -= 32;
-                const uint32_t ent = q[qn + lane];
-                const uint32_t j0 = ent >> 16, k1 = ent & 0xFFFFu;
-                const uint32_t t = count_h2(sm, cell, ncell, c, sm.sx[j0], sm.sy[j0], __ldg(x + b1 + k1),
-                                            __ldg(y + b1 + k1), kmin, R, sh, nb);
-                if (t) atomicAdd(&sm.m[k1], t);
-                __syncwarp();
+          }
+          trip += t;
+          // a6: middle hits with triplets -> the station's list (distinct hits: every h1 has one lane)
+          const uint32_t am = __ballot_sync(FULL, t != 0);
+          if (am && !dead) {
+            const int leader = __ffs(am) - 1;
+            uint32_t pos = 0;
+            if ((int)lane == leader) pos = atomicAdd(&sm.ucount[sp], (uint32_t)__popc(am));
+            pos = __shfl_sync(FULL, pos, leader) + __popc(am & lanemask_lt());
+            if (t) {
+              if (pos < (uint32_t)LISTCAP) {
+                sm.ux[cur][pos] = x1; sm.uy[cur][pos] = y1; sm.uc[cur][pos] = t;
+              } else {
+                const uint32_t o = pos - LISTCAP;
+                spill_i[(cur * 3 + 0) * CAP + o] = x1; spill_i[(cur * 3 + 1) * CAP + o] = y1;
+                spill_cta[(cur * 3 + 2) * CAP + o] = t;
               }
             }
           }
         }
-        __syncwarp();
-        if (lane < qn) {
-          const uint32_t ent = q[lane];
-          const uint32_t j0 = ent >> 16, k1 = ent & 0xFFFFu;
-          const uint32_t t = count_h2(sm, cell, ncell, c, sm.sx[j0], sm.sy[j0], __ldg(x + b1 + k1), __ldg(y + b1 + k1),
-                                      kmin, R, sh, nb);
-          if (t) atomicAdd(&sm.m[k1], t);
+        if (__any_sync(FULL, trip != 0)) {
+#pragma unroll
+          for (int d = 16; d >= 1; d >>= 1) trip += __shfl_xor_sync(FULL, trip, d);
+          if (lane == 0) atomicAdd(&sm.acc[sp], trip);
         }
+      }
+      team_sync<W>();
+
+      // ---- F: the search is over: the staging buffer, the chains and the bitmaps are free
+      const uint32_t ncur = dead ? 0u : sm.ucount[sp];
+      if (tid == 0) {
+        n_triplets[(size_t)e * S + s] = sat32(sm.acc[sp]);
+        sm.acc[sp ^ 1u] = 0;
+        sm.nsurv[sp ^ 1u] = 0;
+        sm.ucount[sp ^ 1u] = 0;
+        if (s + 1 < S && searchable(s + 1)) issue_stage(s + 1);
+      }
+      if (search) {
+        uint4* const v = reinterpret_cast<uint4*>(sm.head);
+        for (uint32_t i = tid; i < kZeroVec; i += T) v[i] = make_uint4(0, 0, 0, 0);
       }
       if (s == 0 && pf_b > pf_a) {  // pull the next event of this team into L2 while this one is being searched
         const uint32_t la = pf_a >> 5, lb = (pf_b + 31) >> 5;  // 128-byte lines
@@ -520,42 +594,8 @@ __global__ void __launch_bounds__(32 * W, MINB)
           prefetch_l2(y + (size_t)l * 32);
         }
       }
-      team_sync<W>();
-
-      // ---- station total, list of distinct middle hits with triplets (R8)
-      if (search) {
-        constexpr bool kSmallSum = (CAP + T - 1) / T < 8;  // 32 lanes * 7 hits * 2^24 < 2^32
-        uint32_t part32 = 0;
-        unsigned long long part64 = 0;
-        for (uint32_t i = tid; i < n1; i += T) {
-          const uint32_t mm = sm.m[i];
-          if (kSmallSum) part32 += mm; else part64 += mm;
-          if (mm && !dead) {
-            const uint32_t pos = atomicAdd(&sm.ucount, 1u);
-            const int32_t hx = __ldg(x + b1 + i), hy = __ldg(y + b1 + i);
-            if (pos < (uint32_t)LISTCAP) {
-              sm.ux[cur][pos] = hx; sm.uy[cur][pos] = hy; sm.uc[cur][pos] = mm;
-            } else {
-              const uint32_t o = pos - LISTCAP;
-              spill_i[(cur * 3 + 0) * CAP + o] = hx; spill_i[(cur * 3 + 1) * CAP + o] = hy;
-              spill_cta[(cur * 3 + 2) * CAP + o] = mm;
-            }
-          }
-        }
-        if (kSmallSum) {
-          part32 = __reduce_add_sync(0xFFFFFFFFu, part32);
-          if (lane == 0 && part32) atomicAdd(&sm.acc, (unsigned long long)part32);
-        } else {
-#pragma unroll
-          for (int d = 16; d >= 1; d >>= 1) part64 += __shfl_xor_sync(0xFFFFFFFFu, part64, d);
-          if (lane == 0 && part64) atomicAdd(&sm.acc, part64);
-        }
-      }
-      team_sync<W>();
-      const uint32_t ncur = dead ? 0u : sm.ucount;
-      if (tid == 0) n_triplets[(size_t)e * S + s] = sat32(sm.acc);
       // ---- a7: chain counts c_s[u] = m_u * sum over linked t of c_{s-1}[t], saturating (R9)
-      if (s > 0 && !dead && ncur) {
+      if (s > 0 && ncur) {
         const int32_t nzA = -p.z[3 * (s - 1) + 1], zB = c.z1;
         const int64_t TL = p.thr_link[s];
         const uint64_t TLx2 = p.thr2_link[s];
@@ -589,29 +629,24 @@ __global__ void __launch_bounds__(32 * W, MINB)
       if (ncur == 0) dead = true;
       nprev = ncur;
       cur ^= 1;
+      sp ^= 1u;
       team_sync<W>();
     }
 
     // ---- candidates = sum over the last station's middle hits; a8: one writer per event
-    if (tid == 0) sm.acc = 0;
-    team_sync<W>();
-    if (!dead) {
+    if (warp == 0) {
       unsigned long long part = 0;
-      for (uint32_t u = tid; u < nprev; u += T)
-        part += u < (uint32_t)LISTCAP ? sm.uc[cur ^ 1][u] : spill_cta[((cur ^ 1) * 3 + 2) * CAP + u - LISTCAP];
-      if (__any_sync(0xFFFFFFFFu, part != 0)) {
+      if (!dead)
+        for (uint32_t u = lane; u < nprev; u += 32)
+          part += u < (uint32_t)LISTCAP ? sm.uc[cur ^ 1][u] : spill_cta[((cur ^ 1) * 3 + 2) * CAP + u - LISTCAP];
 #pragma unroll
-        for (int d = 16; d >= 1; d >>= 1) part += __shfl_xor_sync(0xFFFFFFFFu, part, d);
-        if (lane == 0) atomicAdd(&sm.acc, part);
+      for (int d = 16; d >= 1; d >>= 1) part += __shfl_xor_sync(FULL, part, d);
+      if (lane == 0) {
+        const uint32_t cand = sat32(part);
+        n_candidates[e] = cand;
+        accept[e] = cand >= p.min_candidates ? 1 : 0;
       }
     }
-    team_sync<W>();
-    if (tid == 0) {
-      const uint32_t cand = sat32(sm.acc);
-      n_candidates[e] = cand;
-      accept[e] = cand >= p.min_candidates ? 1 : 0;
-    }
-    team_sync<W>();
   }
 }
 

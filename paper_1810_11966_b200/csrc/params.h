@@ -26,13 +26,14 @@ struct Params {
   // the same thresholds doubled: the test is evaluated as (uint64)(a*z_B + T - b*z_A) <= 2*T
   uint64_t thr2_in[kMaxStations][3];
   uint64_t thr2_link[kMaxStations];
-  // slope keys used ONLY to choose which bins to look at (never to accept or reject a pair):
+  // slope keys used ONLY to choose which cells to look at (never to accept or reject a pair):
   // key(x, l) = mulhi(x, key_mul[l]) = floor(x * key_mul[l] / 2^32) ~ K * x / z_l, with |key - K*x/z_l| < 1.25
   int32_t key_mul[kMaxLayers];
   int32_t key_min;                     // key of slope -slope_range
   int32_t key_R;                       // two x- (or y-) compatible hits have |key_h - key_g| <= key_R
-  int32_t cls_shift[kNumTeamClasses];  // bin = clamp((key - key_min) >> shift, 0, nb-1); 2*key_R <= 2^shift
-  uint32_t cls_nb[kNumTeamClasses];    // bins per axis (grid is nb x nb per layer)
+  // fine cell = clamp((key - key_min) >> fsh, 0, nf-1), key_R <= 2^fsh; coarse cell = fine cell >> 1
+  int32_t cls_fsh[kNumTeamClasses];
+  uint32_t cls_nf[kNumTeamClasses];    // fine cells per axis (1, 2, 4, ... 64); coarse cells per axis = max(nf/2, 1)
   uint32_t cls_max[kNumTeamClasses];   // fullest layer an event of this class may have
   uint32_t min_candidates;
   uint32_t max_hits_per_layer;
