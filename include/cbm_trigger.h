@@ -73,8 +73,7 @@ typedef struct {
   uint32_t n_slots;                    /* 0..4 slots of (pinned host + device) buffers; 2 = double buffering.
                                           0: only cbm_trigger_run_device() is usable (caller owns all buffers) */
   int32_t  device;                     /* CUDA ordinal */
-  uint32_t slope_range_milli;          /* tuning hint, never changes results: hits are binned over slopes
-                                          |x/z|,|y/z| <= this/1000 (outliers share the edge bins). 0 = 400 */
+  uint32_t slope_range_milli;          /* ignored (kept for ABI layout): the slope grid is cyclic and needs no range */
   uint32_t tiny_max_layer_hits;        /* tuning: events whose fullest layer holds <= this many hits (and that fit
                                           the tile) take the thread-per-station path. 0 = default (24); max 32 */
   uint32_t flags;                      /* CBM_FLAG_* */

@@ -157,30 +157,26 @@ int build_params(const cbm_trigger_config_t& c, Params& p, std::string& why) {
   // Slope keys: key = floor(x*M_l/2^32), M_l = round(2^32*K/z_l) < 2^31.
   // For any int32 x: |x*M_l/2^32 - K*x/z_l| <= 2^31 * 0.5/2^32 = 0.25, floor loses < 1  =>  |key - K*x/z_l| < 1.25.
   // Two hits with |x_h/z_A - x_g/z_B| <= w therefore have |key_h - key_g| < w*K + 2.5 <= R := ceil(w*K) + 3.
-  // Grid: nf fine cells of 2^fsh keys per axis cover the slope range (outliers share the edge cells); a fine
-  // cell must be at least R wide (compatible hits lie in fine cells at most one apart; a coarse cell = two fine
-  // cells >= 2R, so a window touches at most 2 x 2 coarse cells).  Largest nf first, then the largest K.
+  // Grid: fine cell = floor(key / 2^fsh) mod nf (cyclic, so no slope range has to be covered), 2^fsh >= R:
+  // compatible hits lie in fine cells at most one apart; a coarse cell = two fine cells >= 2R, so a window
+  // touches at most 2 x 2 coarse cells.  K is chosen so that the fine cell is as narrow as the window allows.
   const double w = (double)c.win_in_num / (double)c.win_in_den;
-  const double smax = (c.slope_range_milli ? c.slope_range_milli : 400) / 1000.0;
   const double Kmax = 0.499 * (double)p.z[0];
-  int nf = 1, fsh = 30, R = 0;
-  double K = Kmax;
-  bool ok = false;
-  for (int n = kNfH; n >= 2 && !ok; n >>= 1) {
-    for (int sh = 14; sh >= 2 && !ok; --sh) {
-      const double k = ((double)n * std::ldexp(1.0, sh) - 2.0) / (2.0 * smax);  // n * 2^sh keys span the range
-      if (k > Kmax || k < 4.0) continue;
-      const int r = (int)std::ceil(w * k) + 3;
-      if (r <= (1 << sh)) { ok = true; nf = n; fsh = sh; K = k; R = r; }
-    }
+  int fsh = 2, R = 3;
+  double K = 0, best = 1e300;
+  for (int sh = 2; sh <= 14; ++sh) {
+    const double two = std::ldexp(1.0, sh);
+    const double k = w > 0 ? std::min(Kmax, (two - 3.0) / w * (1.0 - 1e-9)) : Kmax;
+    if (k <= 0) continue;
+    const int r = (int)std::ceil(w * k) + 3;
+    if (r <= (1 << sh) && two / k < best) { best = two / k; fsh = sh; K = k; R = r; }
   }
-  // !ok: geometry too fine for the key resolution: one cell per layer (still exact, just slower)
+  if (K <= 0) { why = "internal: no slope key scale"; return CBM_ERR_INVALID_ARG; }
   p.key_R = R;
-  p.key_min = ok ? -(int)std::ceil(smax * K) : 0;
-  p.cls_nf[kClsH] = p.cls_nf[kClsG] = (uint32_t)nf;
+  p.cls_nf[kClsH] = p.cls_nf[kClsG] = (uint32_t)kNfH;
   p.cls_fsh[kClsH] = p.cls_fsh[kClsG] = fsh;
-  if (nf >= 2) { p.cls_nf[kClsM] = (uint32_t)std::min(nf / 2, kNfM); p.cls_fsh[kClsM] = fsh + (nf / 2 <= kNfM ? 1 : 2); }
-  else { p.cls_nf[kClsM] = 1; p.cls_fsh[kClsM] = fsh; }
+  p.cls_nf[kClsM] = (uint32_t)kNfM;  // fewer hits per layer: cells twice as wide
+  p.cls_fsh[kClsM] = fsh + 1;
   for (uint32_t l = 0; l < p.L; ++l) {
     const double m = std::ldexp(K, 32) / (double)p.z[l];
     const long long mi = llround(m);

@@ -284,8 +284,16 @@ struct TeamSmem {
   alignas(8) uint64_t bar;                    // completion of the station's bulk copies
 };
 
-__device__ __forceinline__ int bin_of(int key, int kmin, int sh, int nbm1) {
-  return min(max((key - kmin) >> sh, 0), nbm1);
+// fine cell of a slope key on the cyclic grid: floor(key / 2^sh) mod nf (nf a power of two, mask = nf - 1).
+// Keys outside the covered range alias onto other cells; that only adds candidates, never loses one.
+__device__ __forceinline__ uint32_t cell_of(int key, int sh, uint32_t mask) { return (uint32_t)(key >> sh) & mask; }
+
+// shared-memory atomic add issued by exactly one lane (a warp-aggregated count): plain ATOMS, the compiler
+// must not wrap it in its own warp aggregation
+__device__ __forceinline__ uint32_t atoms_add(uint32_t* addr, uint32_t v) {
+  uint32_t old;
+  asm volatile("atom.shared.add.u32 %0, [%1], %2;" : "=r"(old) : "r"(smem_u32(addr)), "r"(v) : "memory");
+  return old;
 }
 
 __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
@@ -304,32 +312,31 @@ struct StationConst {
   uint64_t T01x2, T02x2, T12x2;
 };
 
-// Chain heads of the <= 2x2 coarse cells that can hold a hit compatible with a hit whose window starts in
-// `cell` (dx / dy: the window reaches the next cell row / column); non-empty heads first.
-struct Heads { uint32_t a, b, c, d; };
-__device__ __forceinline__ Heads load_heads(const uint32_t* head, uint32_t cell, bool dx, bool dy, int nc) {
-  Heads h;
-  h.a = head[cell];
-  h.b = dy ? head[cell + 1] : 0u;
-  h.c = dx ? head[cell + nc] : 0u;
-  h.d = (dx && dy) ? head[cell + nc + 1] : 0u;
-  if (!h.c) { h.c = h.d; h.d = 0; }
-  if (!h.b) { h.b = h.c; h.c = h.d; h.d = 0; }
-  if (!h.a) { h.a = h.b; h.b = h.c; h.c = h.d; h.d = 0; }
-  return h;
+// Chain heads (index + 1 <= 4096, 16 bits each) of the <= 2x2 coarse cells that can hold a hit compatible with
+// a hit whose window covers rows lox..hix and columns loy..hiy (cyclic); non-empty heads only, packed from bit 0.
+__device__ __forceinline__ unsigned long long load_heads(const uint32_t* head, uint32_t lox, uint32_t hix, uint32_t loy,
+                                                         uint32_t hiy, uint32_t nc) {
+  unsigned long long hq = 0;
+  const bool dx = hix != lox, dy = hiy != loy;
+  uint32_t v = head[lox * nc + loy];
+  if (v) hq = v;
+  if (dy) { v = head[lox * nc + hiy]; if (v) hq = (hq << 16) | v; }
+  if (dx) { v = head[hix * nc + loy]; if (v) hq = (hq << 16) | v; }
+  if (dx && dy) { v = head[hix * nc + hiy]; if (v) hq = (hq << 16) | v; }
+  return hq;
 }
 
 // Rare path of phase D (a middle hit with more than three compatible h0): number of h0 in the <= 2x2 cells
 // compatible with both h1 (anchors Qx, Qy) and h2 (x2, y2).  No warp-level operation inside.
 template <class SM>
-__device__ __noinline__ uint32_t count_h0_slow(const SM& sm, const uint32_t* head, uint32_t o0, uint32_t cell, bool dx,
-                                               bool dy, int nc, const StationConst& c, int64_t Qx, int64_t Qy, int32_t x2,
-                                               int32_t y2) {
+__device__ __noinline__ uint32_t count_h0_slow(const SM& sm, const uint32_t* head, uint32_t o0, uint32_t lox, uint32_t hix,
+                                               uint32_t loy, uint32_t hiy, uint32_t nc, const StationConst& c, int64_t Qx,
+                                               int64_t Qy, int32_t x2, int32_t y2) {
   uint32_t n = 0;
   for (int q = 0; q < 4; ++q) {
-    if ((q & 1) && !dy) continue;
-    if ((q & 2) && !dx) continue;
-    for (uint32_t cur = head[cell + (q & 1) + ((q & 2) ? nc : 0)]; cur; cur = sm.next[0][cur - 1]) {
+    if ((q & 1) && hiy == loy) continue;
+    if ((q & 2) && hix == lox) continue;
+    for (uint32_t cur = head[((q & 2) ? hix : lox) * nc + ((q & 1) ? hiy : loy)]; cur; cur = sm.next[0][cur - 1]) {
       const int32_t x0 = sm.sx[o0 + cur - 1], y0 = sm.sy[o0 + cur - 1];
       const bool ok = win_q(x0, c.z1, Qx, c.T01x2) & win_q(y0, c.z1, Qy, c.T01x2) &
                       win_q(x2, c.z0, anchor_q(x0, c.nz2, c.T02), c.T02x2) &
@@ -357,9 +364,9 @@ __global__ void __launch_bounds__(32 * W, MINB)
   const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const uint32_t S = p.S, L = p.L;
   const uint32_t n_list = ctrl->count[CLS];
-  const int kmin = p.key_min, R = p.key_R, fsh = p.cls_fsh[CLS], csh = fsh + 1;
-  const int nf1 = (int)p.cls_nf[CLS] - 1;
-  const int nc = max((int)p.cls_nf[CLS] >> 1, 1), nc1 = nc - 1;
+  const int R = p.key_R, fsh = p.cls_fsh[CLS], csh = fsh + 1;
+  const uint32_t nf = p.cls_nf[CLS], nf1 = nf - 1u;
+  const uint32_t nc = max(nf >> 1, 1u), nc1 = nc - 1u;
   uint32_t* const head0 = sm.head;
   uint32_t* const head2 = sm.head + nc * nc;
   // spill area of this CTA: list entries beyond LISTCAP, [2 lists][x, y, c][CAP] words
@@ -382,6 +389,9 @@ __global__ void __launch_bounds__(32 * W, MINB)
   team_sync<W>();
   uint32_t par = 0;  // phase parity of the staging barrier
   uint32_t sp = 0;   // parity of the per-station counters
+  // Warp w of every resident CTA sits on scheduler w % 4, and phases B..D give the low warps more work
+  // (row 0..63, the first 32-chunks): the roles rotate from station to station so that the schedulers even out.
+  uint32_t rot = 0;
 
   // a4: thread 0 starts the bulk copies of station s of the event whose offsets are in sm.off
   auto searchable = [&](uint32_t s) {
@@ -426,33 +436,45 @@ __global__ void __launch_bounds__(32 * W, MINB)
       c.T01 = p.thr_in[s][0]; c.T02 = p.thr_in[s][1]; c.T12 = p.thr_in[s][2];
       c.T01x2 = p.thr2_in[s][0]; c.T02x2 = p.thr2_in[s][1]; c.T12x2 = p.thr2_in[s][2];
       const bool search = (n0 != 0) & (n1 != 0) & (n2 != 0);
+      const uint32_t vwarp = (warp + rot) & (W - 1), vtid = vwarp * 32 + lane;
+      rot = (rot + 1u) & (W - 1);
       if (search) {
         while (!mbar_try_wait(&sm.bar, par)) {
         }
         par ^= 1u;
-        // ---- A: chains of layers 0 and 2 on the coarse grid, fine occupancy bitmaps
-        for (uint32_t i = tid; i < n0 + n2; i += T) {
-          const bool l2 = i >= n0;
-          const uint32_t j = l2 ? i - n0 : i;
-          const uint32_t si = (l2 ? o2 : o0) + j;
-          const int32_t M = l2 ? c.M2 : c.M0;
-          const int fx = bin_of(__mulhi(sm.sx[si], M), kmin, fsh, nf1), fy = bin_of(__mulhi(sm.sy[si], M), kmin, fsh, nf1);
-          uint32_t* const hd = l2 ? head2 : head0;
-          const uint32_t old = atomicExch(&hd[(fx >> 1) * nc + (fy >> 1)], j + 1u);
-          sm.next[l2 ? 1 : 0][j] = (uint16_t)old;
-          atomicOr(&sm.occ[l2 ? 1 : 0][2 * fx + (fy >> 5)], 1u << (fy & 31));
+        // ---- A: chains of layers 0 and 2 on the coarse grid, fine occupancy bitmaps.  The first half of the
+        // team's warps takes layer 0, the second half layer 2 (one warp: both in turn).
+        {
+          constexpr uint32_t TH = W > 1 ? T / 2 : T;
+#pragma unroll 1
+          for (int pass = 0; pass < (W > 1 ? 1 : 2); ++pass) {
+            const int l = W > 1 ? (int)(tid >= TH) : pass;  // 0: layer 0, 1: layer 2  (warp-uniform)
+            const uint32_t n = l ? n2 : n0;
+            const int32_t* const px = sm.sx + (l ? o2 : o0);
+            const int32_t* const py = sm.sy + (l ? o2 : o0);
+            const int32_t M = l ? c.M2 : c.M0;
+            uint32_t* const hd = l ? head2 : head0;
+            uint32_t* const oc = sm.occ[l];
+            uint16_t* const nx = sm.next[l];
+            for (uint32_t j = W > 1 ? tid - (l ? TH : 0u) : tid; j < n; j += TH) {
+              const uint32_t fx = cell_of(__mulhi(px[j], M), fsh, nf1), fy = cell_of(__mulhi(py[j], M), fsh, nf1);
+              const uint32_t old = atomicExch(&hd[(fx >> 1) * nc + (fy >> 1)], j + 1u);
+              nx[j] = (uint16_t)old;
+              atomicOr(&oc[2 * fx + (fy >> 5)], 1u << (fy & 31));
+            }
+          }
         }
         team_sync<W>();
-        // ---- B: J = dilate(occ0) & dilate(occ2); a compatible pair lies in fine cells at most one apart
-        for (uint32_t r = tid; r < 64; r += T) {
+        // ---- B: J = dilate(occ0) & dilate(occ2) on the cyclic grid; a compatible pair lies in fine cells at
+        // most one apart in x and in y
+        for (uint32_t r = vtid; r < nf; r += T) {
+          const unsigned long long full = nf == 64 ? ~0ull : ((1ull << nf) - 1ull);
           unsigned long long d[2];
 #pragma unroll
           for (int l = 0; l < 2; ++l) {
             const unsigned long long* rows = reinterpret_cast<const unsigned long long*>(sm.occ[l]);
-            unsigned long long v = rows[r];
-            if (r > 0) v |= rows[r - 1];
-            if (r < 63) v |= rows[r + 1];
-            d[l] = v | (v << 1) | (v >> 1);
+            const unsigned long long v = rows[r] | rows[(r - 1u) & nf1] | rows[(r + 1u) & nf1];
+            d[l] = (v | (v << 1) | (v >> nf1) | (v >> 1) | (v << nf1)) & full;
           }
           const unsigned long long j = d[0] & d[1];
           sm.J[2 * r] = (uint32_t)j;
@@ -460,19 +482,19 @@ __global__ void __launch_bounds__(32 * W, MINB)
         }
         team_sync<W>();
         // ---- C (a6): middle hits whose fine cell is in J, compacted with ballot/popc
-        for (uint32_t base = warp * 32; base < n1; base += T) {
+        for (uint32_t base = vwarp * 32; base < n1; base += T) {
           const uint32_t i1 = base + lane;
           bool keep = false;
           if (i1 < n1) {
-            const int fx = bin_of(__mulhi(sm.sx[o1 + i1], c.M1), kmin, fsh, nf1);
-            const int fy = bin_of(__mulhi(sm.sy[o1 + i1], c.M1), kmin, fsh, nf1);
+            const uint32_t fx = cell_of(__mulhi(sm.sx[o1 + i1], c.M1), fsh, nf1);
+            const uint32_t fy = cell_of(__mulhi(sm.sy[o1 + i1], c.M1), fsh, nf1);
             keep = (sm.J[2 * fx + (fy >> 5)] >> (fy & 31)) & 1u;
           }
           const uint32_t km = __ballot_sync(FULL, keep);
           if (km) {
             const int leader = __ffs(km) - 1;
             uint32_t pos = 0;
-            if ((int)lane == leader) pos = atomicAdd(&sm.nsurv[sp], (uint32_t)__popc(km));
+            if ((int)lane == leader) pos = atoms_add(&sm.nsurv[sp], (uint32_t)__popc(km));
             pos = __shfl_sync(FULL, pos, leader);
             if (keep) sm.surv[pos + __popc(km & lanemask_lt())] = (uint16_t)i1;
           }
@@ -481,69 +503,66 @@ __global__ void __launch_bounds__(32 * W, MINB)
         // ---- D (a5): one lane per surviving middle hit
         const uint32_t nsv = sm.nsurv[sp];
         unsigned long long trip = 0;
-        for (uint32_t cb = warp * 32; cb < nsv; cb += T) {
+        for (uint32_t cb = vwarp * 32; cb < nsv; cb += T) {
           const bool act = cb + lane < nsv;
           int32_t x1 = 0, y1 = 0;
-          uint32_t cell = 0;
-          bool dx = false, dy = false;
-          Heads h = {0, 0, 0, 0};
+          uint32_t lox = 0, hix = 0, loy = 0, hiy = 0;
+          unsigned long long hq = 0;  // chain heads still to walk (16 bits each)
           if (act) {
             const uint32_t i1 = sm.surv[cb + lane];
             x1 = sm.sx[o1 + i1];
             y1 = sm.sy[o1 + i1];
-            const int tx = __mulhi(x1, c.M1) - R - kmin, ty = __mulhi(y1, c.M1) - R - kmin;
-            const int lox = min(max(tx >> csh, 0), nc1), hix = min(max((tx + 2 * R) >> csh, 0), nc1);
-            const int loy = min(max(ty >> csh, 0), nc1), hiy = min(max((ty + 2 * R) >> csh, 0), nc1);
-            cell = (uint32_t)(lox * nc + loy);
-            dx = hix != lox;
-            dy = hiy != loy;
-            h = load_heads(head0, cell, dx, dy, nc);
+            const int kx = __mulhi(x1, c.M1), ky = __mulhi(y1, c.M1);
+            lox = cell_of(kx - R, csh, nc1); hix = cell_of(kx + R, csh, nc1);
+            loy = cell_of(ky - R, csh, nc1); hiy = cell_of(ky + R, csh, nc1);
+            hq = load_heads(head0, lox, hix, loy, hiy, nc);
           }
           // h0 compatible with h1:  |x0*z1 - x1*z0| <= T01  <=>  (uint64)(x0*z1 + (T01 - x1*z0)) <= 2*T01
           const int64_t Qx = anchor_q(x1, c.nz0, c.T01), Qy = anchor_q(y1, c.nz0, c.T01);
-          uint32_t np = 0, p0 = 0, p1 = 0, p2 = 0;  // number of compatible h0, the first three (index + 1)
-          uint32_t cu = h.a;
+          uint32_t np = 0, pk = 0;  // number of compatible h0; the first two (index + 1, 16 bits each)
+          uint32_t cu = (uint32_t)hq & 0xFFFFu;
+          hq >>= 16;
           while (__any_sync(FULL, cu != 0)) {
             if (cu) {
               const uint32_t j = cu - 1u;
               const int32_t x0 = sm.sx[o0 + j], y0 = sm.sy[o0 + j];
               const uint32_t nx = sm.next[0][j];
               if (win_q(x0, c.z1, Qx, c.T01x2) & win_q(y0, c.z1, Qy, c.T01x2)) {
-                if (np == 0) p0 = cu; else if (np == 1) p1 = cu; else if (np == 2) p2 = cu;
+                if (np < 2) pk |= cu << (np << 4);
                 ++np;
               }
               cu = nx;
-              if (!cu) { cu = h.b; h.b = h.c; h.c = h.d; h.d = 0; }
+              if (!cu) { cu = (uint32_t)hq & 0xFFFFu; hq >>= 16; }
             }
           }
           uint32_t t = 0;  // triplets with this middle hit
           if (__any_sync(FULL, np != 0)) {
-            Heads g = {0, 0, 0, 0};
-            if (np) g = load_heads(head2, cell, dx, dy, nc);
+            hq = np ? load_heads(head2, lox, hix, loy, hiy, nc) : 0ull;
             // h2 compatible with h1:  |x2*z1 - x1*z2| <= T12;  with h0:  |x2*z0 - x0*z2| <= T02
             const int64_t Rx = anchor_q(x1, c.nz2, c.T12), Ry = anchor_q(y1, c.nz2, c.T12);
-            cu = g.a;
+            cu = (uint32_t)hq & 0xFFFFu;
+            hq >>= 16;
             while (__any_sync(FULL, cu != 0)) {
               if (cu) {
                 const uint32_t j = cu - 1u;
                 const int32_t x2 = sm.sx[o2 + j], y2 = sm.sy[o2 + j];
                 const uint32_t nx = sm.next[1][j];
                 if (win_q(x2, c.z1, Rx, c.T12x2) & win_q(y2, c.z1, Ry, c.T12x2)) {
-                  if (np <= 3) {
-                    uint32_t pk = p0;
-                    for (uint32_t k = 0; k < np; ++k) {
-                      const int32_t x0 = sm.sx[o0 + pk - 1u], y0 = sm.sy[o0 + pk - 1u];
+                  if (np <= 2) {
+                    uint32_t q = pk;
+                    do {
+                      const int32_t x0 = sm.sx[o0 + (q & 0xFFFFu) - 1u], y0 = sm.sy[o0 + (q & 0xFFFFu) - 1u];
                       const bool ok = win_q(x2, c.z0, anchor_q(x0, c.nz2, c.T02), c.T02x2) &
                                       win_q(y2, c.z0, anchor_q(y0, c.nz2, c.T02), c.T02x2);
                       t += ok ? 1u : 0u;
-                      pk = k == 0 ? p1 : p2;
-                    }
+                      q >>= 16;
+                    } while (q);
                   } else {
-                    t += count_h0_slow(sm, head0, o0, cell, dx, dy, nc, c, Qx, Qy, x2, y2);
+                    t += count_h0_slow(sm, head0, o0, lox, hix, loy, hiy, nc, c, Qx, Qy, x2, y2);
                   }
                 }
                 cu = nx;
-                if (!cu) { cu = g.b; g.b = g.c; g.c = g.d; g.d = 0; }
+                if (!cu) { cu = (uint32_t)hq & 0xFFFFu; hq >>= 16; }
               }
             }
           }
@@ -553,7 +572,7 @@ __global__ void __launch_bounds__(32 * W, MINB)
           if (am && !dead) {
             const int leader = __ffs(am) - 1;
             uint32_t pos = 0;
-            if ((int)lane == leader) pos = atomicAdd(&sm.ucount[sp], (uint32_t)__popc(am));
+            if ((int)lane == leader) pos = atoms_add(&sm.ucount[sp], (uint32_t)__popc(am));
             pos = __shfl_sync(FULL, pos, leader) + __popc(am & lanemask_lt());
             if (t) {
               if (pos < (uint32_t)LISTCAP) {

@@ -29,11 +29,10 @@ struct Params {
   // slope keys used ONLY to choose which cells to look at (never to accept or reject a pair):
   // key(x, l) = mulhi(x, key_mul[l]) = floor(x * key_mul[l] / 2^32) ~ K * x / z_l, with |key - K*x/z_l| < 1.25
   int32_t key_mul[kMaxLayers];
-  int32_t key_min;                     // key of slope -slope_range
   int32_t key_R;                       // two x- (or y-) compatible hits have |key_h - key_g| <= key_R
-  // fine cell = clamp((key - key_min) >> fsh, 0, nf-1), key_R <= 2^fsh; coarse cell = fine cell >> 1
+  // fine cell = floor(key / 2^fsh) mod nf (cyclic grid), key_R <= 2^fsh; coarse cell = fine cell >> 1
   int32_t cls_fsh[kNumTeamClasses];
-  uint32_t cls_nf[kNumTeamClasses];    // fine cells per axis (1, 2, 4, ... 64); coarse cells per axis = max(nf/2, 1)
+  uint32_t cls_nf[kNumTeamClasses];    // fine cells per axis (power of two <= 64); coarse cells per axis = max(nf/2, 1)
   uint32_t cls_max[kNumTeamClasses];   // fullest layer an event of this class may have
   uint32_t min_candidates;
   uint32_t max_hits_per_layer;
