@@ -56,5 +56,6 @@ constexpr int kTileEvents = 32;              // events per CTA of the tile kerne
 constexpr uint32_t kTinyMaxTotal = 96;       // a tiny event holds at most this many hits ...
 constexpr uint32_t kTileHitCap = kTileEvents * kTinyMaxTotal + 32;  // ... so a tile never overflows this (see tile_kernel)
 constexpr uint32_t kTinyMaxLayerLimit = 32;
+constexpr int kTileFound = 64;               // (h0,h1) pairs with triplets a tile links itself; more: class M
 
 }  // namespace cbm
