@@ -42,6 +42,20 @@ __device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity) {
       : "memory");
   return ok != 0;
 }
+// Shared-memory loads by 32-bit shared address (+ compile-time byte offset): the hot loops keep one address
+// register and step it, instead of re-deriving generic addresses.
+template <int OFS = 0>
+__device__ __forceinline__ int32_t lds_s32(uint32_t addr) {
+  int32_t v;
+  asm volatile("ld.shared.s32 %0, [%1+%2];" : "=r"(v) : "r"(addr), "n"(OFS));
+  return v;
+}
+template <int OFS = 0>
+__device__ __forceinline__ uint32_t lds_u16(uint32_t addr) {
+  uint32_t v;
+  asm volatile("{ .reg .u16 t; ld.shared.u16 t, [%1+%2]; cvt.u32.u16 %0, t; }" : "=r"(v) : "r"(addr), "n"(OFS));
+  return v;
+}
 // 1-D TMA bulk copy global -> shared, completion counted in bytes on an mbarrier (SASS: UBLKCP).
 // dst, src 16-byte aligned, bytes a multiple of 16.
 __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
@@ -237,16 +251,21 @@ __global__ void __launch_bounds__(kTileEvents* kMaxStations)
     const uint2 dsc = sm.desc[ow];
     const uint32_t b0 = dsc.x & 0xFFFFu, b1 = dsc.x >> 16, b2 = dsc.y & 0xFFFFu, b3 = dsc.y >> 16;
     const TileStation& k = sm.sc[ow >> 5];
-    const int32_t z0 = k.z0, z1 = k.z1;
+    const int32_t z0 = k.z0, z1 = k.z1, nz0 = -z0;
     const int64_t T01 = k.T01;
-    const int32_t x0 = sm.sx[b0 + i0], y0 = sm.sy[b0 + i0];
+    const uint64_t T01x2 = 2 * (uint64_t)T01;
+    constexpr int kDY = (int)(offsetof(TileSmem, sy) - offsetof(TileSmem, sx));
+    const uint32_t ax = smem_u32(sm.sx);
+    const int32_t x0 = lds_s32(ax + 4 * (b0 + i0)), y0 = lds_s32<kDY>(ax + 4 * (b0 + i0));
+    // |x0*z1 - x1*z0| <= T01  <=>  (uint64)(x1*(-z0) + (x0*z1 + T01)) <= 2*T01
     const int64_t Px = (int64_t)x0 * z1 + T01, Py = (int64_t)y0 * z1 + T01;
     uint32_t cnt = 0;
-    for (uint32_t i1 = b1; i1 < b2; ++i1) {
-      const int32_t x1 = sm.sx[i1];
-      if (win(Px, x1, z0, 2 * (uint64_t)T01)) {
-        const int32_t y1 = sm.sy[i1];
-        if (win(Py, y1, z0, 2 * (uint64_t)T01)) {
+    const uint32_t a_end = ax + 4 * b2;
+    for (uint32_t a1 = ax + 4 * b1; a1 != a_end; a1 += 4) {
+      const int32_t x1 = lds_s32(a1);
+      if ((uint64_t)((int64_t)x1 * nz0 + Px) <= T01x2) {
+        const int32_t y1 = lds_s32<kDY>(a1);
+        if ((uint64_t)((int64_t)y1 * nz0 + Py) <= T01x2) {
           const int32_t z2 = k.z2;
           const int64_t T02 = k.T02, T12 = k.T12;
           const int64_t Qx0 = (int64_t)x0 * z2 + T02, Qy0 = (int64_t)y0 * z2 + T02;
@@ -262,7 +281,7 @@ __global__ void __launch_bounds__(kTileEvents* kMaxStations)
             cnt += t;
             const uint32_t slot = atomicAdd(&sm.nfound, 1u);
             if (slot < (uint32_t)kTileFound) {
-              sm.f_key[slot] = (ow << 16) | i1;
+              sm.f_key[slot] = (ow << 16) | ((a1 - ax) >> 2);
               sm.f_t[slot] = t;
             }
           }
