@@ -56,6 +56,22 @@ __device__ __forceinline__ uint32_t lds_u16(uint32_t addr) {
   asm volatile("{ .reg .u16 t; ld.shared.u16 t, [%1+%2]; cvt.u32.u16 %0, t; }" : "=r"(v) : "r"(addr), "n"(OFS));
   return v;
 }
+__device__ __forceinline__ uint32_t lds_u32(uint32_t addr) {
+  uint32_t v;
+  asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr));
+  return v;
+}
+__device__ __forceinline__ void sts_u16(uint32_t addr, uint32_t v) {
+  asm volatile("{ .reg .u16 t; cvt.u16.u32 t, %1; st.shared.u16 [%0], t; }" ::"r"(addr), "r"(v) : "memory");
+}
+__device__ __forceinline__ uint32_t atoms_exch(uint32_t addr, uint32_t v) {
+  uint32_t old;
+  asm volatile("atom.shared.exch.b32 %0, [%1], %2;" : "=r"(old) : "r"(addr), "r"(v) : "memory");
+  return old;
+}
+__device__ __forceinline__ void reds_or(uint32_t addr, uint32_t v) {
+  asm volatile("red.shared.or.b32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
+}
 // 1-D TMA bulk copy global -> shared, completion counted in bytes on an mbarrier (SASS: UBLKCP).
 // dst, src 16-byte aligned, bytes a multiple of 16.
 __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
@@ -480,6 +496,9 @@ __global__ void __launch_bounds__(32 * W, MINB)
   const uint32_t nc = max(nf >> 1, 1u), nc1 = nc - 1u;
   uint32_t* const head0 = sm.head;
   uint32_t* const head2 = sm.head + nc * nc;
+  const uint32_t lnc = 31u - (uint32_t)__clz(nc);  // nc = 2^lnc: coarse cell (cx, cy) is head[(cx << lnc) | cy]
+  constexpr int kDY = (int)(offsetof(SM, sy) - offsetof(SM, sx));
+  const uint32_t a_sx = smem_u32(sm.sx);
   // spill area of this CTA: list entries beyond LISTCAP, [2 lists][x, y, c][CAP] words
   uint32_t* const spill_cta = spill + (size_t)blockIdx.x * 6 * CAP;
   int32_t* const spill_i = reinterpret_cast<int32_t*>(spill_cta);
@@ -560,18 +579,17 @@ __global__ void __launch_bounds__(32 * W, MINB)
 #pragma unroll 1
           for (int pass = 0; pass < (W > 1 ? 1 : 2); ++pass) {
             const int l = W > 1 ? (int)(tid >= TH) : pass;  // 0: layer 0, 1: layer 2  (warp-uniform)
-            const uint32_t n = l ? n2 : n0;
-            const int32_t* const px = sm.sx + (l ? o2 : o0);
-            const int32_t* const py = sm.sy + (l ? o2 : o0);
             const int32_t M = l ? c.M2 : c.M0;
-            uint32_t* const hd = l ? head2 : head0;
-            uint32_t* const oc = sm.occ[l];
-            uint16_t* const nx = sm.next[l];
-            for (uint32_t j = W > 1 ? tid - (l ? TH : 0u) : tid; j < n; j += TH) {
-              const uint32_t fx = cell_of(__mulhi(px[j], M), fsh, nf1), fy = cell_of(__mulhi(py[j], M), fsh, nf1);
-              const uint32_t old = atomicExch(&hd[(fx >> 1) * nc + (fy >> 1)], j + 1u);
-              nx[j] = (uint16_t)old;
-              atomicOr(&oc[2 * fx + (fy >> 5)], 1u << (fy & 31));
+            const uint32_t j0 = W > 1 ? tid - (l ? TH : 0u) : tid, n = l ? n2 : n0;
+            uint32_t a_hit = a_sx + 4u * ((l ? o2 : o0) + j0);               // x of hit j; y at + kDY
+            uint32_t a_nx = smem_u32(sm.next[l]) + 2u * j0;
+            const uint32_t a_hd = smem_u32(l ? head2 : head0), a_oc = smem_u32(sm.occ[l]);
+            for (uint32_t j = j0; j < n; j += TH, a_hit += 4u * TH, a_nx += 2u * TH) {
+              const uint32_t fx = cell_of(__mulhi(lds_s32(a_hit), M), fsh, nf1);
+              const uint32_t fy = cell_of(__mulhi(lds_s32<kDY>(a_hit), M), fsh, nf1);
+              const uint32_t old = atoms_exch(a_hd + 4u * (((fx >> 1) << lnc) | (fy >> 1)), j + 1u);
+              sts_u16(a_nx, old);
+              reds_or(a_oc + 4u * ((fx << 1) | (fy >> 5)), 1u << (fy & 31));
             }
           }
         }
@@ -593,13 +611,15 @@ __global__ void __launch_bounds__(32 * W, MINB)
         }
         team_sync<W>();
         // ---- C (a6): middle hits whose fine cell is in J, compacted with ballot/popc
+        const uint32_t a_J = smem_u32(sm.J);
         for (uint32_t base = vwarp * 32; base < n1; base += T) {
           const uint32_t i1 = base + lane;
           bool keep = false;
           if (i1 < n1) {
-            const uint32_t fx = cell_of(__mulhi(sm.sx[o1 + i1], c.M1), fsh, nf1);
-            const uint32_t fy = cell_of(__mulhi(sm.sy[o1 + i1], c.M1), fsh, nf1);
-            keep = (sm.J[2 * fx + (fy >> 5)] >> (fy & 31)) & 1u;
+            const uint32_t a1 = a_sx + 4u * (o1 + i1);
+            const uint32_t fx = cell_of(__mulhi(lds_s32(a1), c.M1), fsh, nf1);
+            const uint32_t fy = cell_of(__mulhi(lds_s32<kDY>(a1), c.M1), fsh, nf1);
+            keep = (lds_u32(a_J + 4u * ((fx << 1) | (fy >> 5))) >> (fy & 31)) & 1u;
           }
           const uint32_t km = __ballot_sync(FULL, keep);
           if (km) {
@@ -614,15 +634,18 @@ __global__ void __launch_bounds__(32 * W, MINB)
         // ---- D (a5): one lane per surviving middle hit
         const uint32_t nsv = sm.nsurv[sp];
         unsigned long long trip = 0;
+        // hit with chain link cu (= index + 1) of layer 0 / 2: x at a_l + 4*cu, y kDY further; its link at a_n + 2*cu
+        const uint32_t a_l0 = a_sx + 4u * o0 - 4u, a_l2 = a_sx + 4u * o2 - 4u;
+        const uint32_t a_n0 = smem_u32(sm.next[0]) - 2u, a_n2 = smem_u32(sm.next[1]) - 2u;
         for (uint32_t cb = vwarp * 32; cb < nsv; cb += T) {
           const bool act = cb + lane < nsv;
           int32_t x1 = 0, y1 = 0;
           uint32_t lox = 0, hix = 0, loy = 0, hiy = 0;
           unsigned long long hq = 0;  // chain heads still to walk (16 bits each)
           if (act) {
-            const uint32_t i1 = sm.surv[cb + lane];
-            x1 = sm.sx[o1 + i1];
-            y1 = sm.sy[o1 + i1];
+            const uint32_t a1 = a_sx + 4u * (o1 + sm.surv[cb + lane]);
+            x1 = lds_s32(a1);
+            y1 = lds_s32<kDY>(a1);
             const int kx = __mulhi(x1, c.M1), ky = __mulhi(y1, c.M1);
             lox = cell_of(kx - R, csh, nc1); hix = cell_of(kx + R, csh, nc1);
             loy = cell_of(ky - R, csh, nc1); hiy = cell_of(ky + R, csh, nc1);
@@ -635,9 +658,8 @@ __global__ void __launch_bounds__(32 * W, MINB)
           hq >>= 16;
           while (__any_sync(FULL, cu != 0)) {
             if (cu) {
-              const uint32_t j = cu - 1u;
-              const int32_t x0 = sm.sx[o0 + j], y0 = sm.sy[o0 + j];
-              const uint32_t nx = sm.next[0][j];
+              const int32_t x0 = lds_s32(a_l0 + 4u * cu), y0 = lds_s32<kDY>(a_l0 + 4u * cu);
+              const uint32_t nx = lds_u16(a_n0 + 2u * cu);
               if (win_q(x0, c.z1, Qx, c.T01x2) & win_q(y0, c.z1, Qy, c.T01x2)) {
                 if (np < 2) pk |= cu << (np << 4);
                 ++np;
@@ -655,14 +677,13 @@ __global__ void __launch_bounds__(32 * W, MINB)
             hq >>= 16;
             while (__any_sync(FULL, cu != 0)) {
               if (cu) {
-                const uint32_t j = cu - 1u;
-                const int32_t x2 = sm.sx[o2 + j], y2 = sm.sy[o2 + j];
-                const uint32_t nx = sm.next[1][j];
+                const int32_t x2 = lds_s32(a_l2 + 4u * cu), y2 = lds_s32<kDY>(a_l2 + 4u * cu);
+                const uint32_t nx = lds_u16(a_n2 + 2u * cu);
                 if (win_q(x2, c.z1, Rx, c.T12x2) & win_q(y2, c.z1, Ry, c.T12x2)) {
                   if (np <= 2) {
                     uint32_t q = pk;
                     do {
-                      const int32_t x0 = sm.sx[o0 + (q & 0xFFFFu) - 1u], y0 = sm.sy[o0 + (q & 0xFFFFu) - 1u];
+                      const int32_t x0 = lds_s32(a_l0 + 4u * (q & 0xFFFFu)), y0 = lds_s32<kDY>(a_l0 + 4u * (q & 0xFFFFu));
                       const bool ok = win_q(x2, c.z0, anchor_q(x0, c.nz2, c.T02), c.T02x2) &
                                       win_q(y2, c.z0, anchor_q(y0, c.nz2, c.T02), c.T02x2);
                       t += ok ? 1u : 0u;
