@@ -751,15 +751,23 @@ __global__ void __launch_bounds__(32 * W, MINB)
         const int64_t TL = p.thr_link[s];
         const uint64_t TLx2 = p.thr2_link[s];
         if (ncur <= (uint32_t)LISTCAP && nprev <= (uint32_t)LISTCAP) {  // everything in shared memory
-          for (uint32_t u = tid; u < ncur; u += T) {
-            // |x_t*zB - x_u*zA| <= TL
-            const int64_t Qx = anchor_q(sm.ux[cur][u], nzA, TL), Qy = anchor_q(sm.uy[cur][u], nzA, TL);
+          // kLinkG lanes share one u: lane g tests the previous station's entries g, g + kLinkG, ...
+          constexpr uint32_t kLinkG = 8;
+          const uint32_t g = tid % kLinkG;
+          for (uint32_t ub = 0; ub < ncur; ub += T / kLinkG) {
+            const uint32_t u = ub + tid / kLinkG;
             unsigned long long a = 0;
-            for (uint32_t t = 0; t < nprev; ++t) {
-              const bool ok = win_q(sm.ux[cur ^ 1][t], zB, Qx, TLx2) & win_q(sm.uy[cur ^ 1][t], zB, Qy, TLx2);
-              if (ok) a += sm.uc[cur ^ 1][t];  // < 4096 * 2^32
+            if (u < ncur) {
+              // |x_t*zB - x_u*zA| <= TL
+              const int64_t Qx = anchor_q(sm.ux[cur][u], nzA, TL), Qy = anchor_q(sm.uy[cur][u], nzA, TL);
+              for (uint32_t t = g; t < nprev; t += kLinkG) {
+                const bool ok = win_q(sm.ux[cur ^ 1][t], zB, Qx, TLx2) & win_q(sm.uy[cur ^ 1][t], zB, Qy, TLx2);
+                if (ok) a += sm.uc[cur ^ 1][t];  // < 4096 * 2^32
+              }
             }
-            sm.uc[cur][u] = sat32((unsigned long long)sat32(a) * sm.uc[cur][u]);  // m_u <= 2^24: no overflow
+#pragma unroll
+            for (int d = kLinkG / 2; d >= 1; d >>= 1) a += __shfl_xor_sync(FULL, a, d);
+            if (u < ncur && g == 0) sm.uc[cur][u] = sat32((unsigned long long)sat32(a) * sm.uc[cur][u]);  // m_u <= 2^24
           }
         } else {  // rare: some entries live in the global spill area
           auto LX = [&](int w, uint32_t i) { return i < (uint32_t)LISTCAP ? sm.ux[w][i] : spill_i[(w * 3 + 0) * CAP + i - LISTCAP]; };
