@@ -189,6 +189,32 @@ def run_reference(args, cfg, cid):
     }))
 
 
+# ---------------------------------------------------------------------------------------------- multi-rank
+def rank_event_range(rank, events_per_rank):
+    """Events are independent: rank r owns the contiguous range
+    [r*E, (r+1)*E) of the synthetic event stream -- weak scaling, no exchange step, no collective
+    in the data path (replicas only)."""
+    return rank * events_per_rank, (rank + 1) * events_per_rank
+
+
+def reduce_over_ranks(dist, device, times, counts):
+    """Whole-job bookkeeping of one bench run: MAX over ranks of every entry of `times` (device
+    time of the slowest rank), SUM over ranks of every entry of `counts` (events, hits).
+    `dist` is torch.distributed or None (single process)."""
+    import torch
+    t = torch.tensor([float(v) for v in times], dtype=torch.float64, device=device)
+    c = torch.tensor([float(v) for v in counts], dtype=torch.float64, device=device)
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dist.all_reduce(c, op=dist.ReduceOp.SUM)
+    return [float(v) for v in t], [float(v) for v in c]
+
+
+def whole_job_rate(total_units, steps, seconds_max):
+    """`value` of the JSON line: units all ranks processed / time of the slowest rank."""
+    return total_units * steps / seconds_max
+
+
 # ---------------------------------------------------------------------------------------------- our arm
 def to_device_padded(torch, a, dev):
     """int32 device copy with the 16-byte tail padding the staging copies may over-read."""
@@ -224,7 +250,7 @@ def run_ours(args, cfg, cid):
     E = args.events or (cfg.chunk_events or cfg.n_events)
     S = cfg.n_stations
     t_gen = time.perf_counter()
-    batch = W.generate(cfg, n_events=E, first_event=rank * E)
+    batch = W.generate(cfg, n_events=E, first_event=rank_event_range(rank, E)[0])
     t_gen = time.perf_counter() - t_gen
     n_hits = batch.n_hits
     B_alg = algorithmic_bytes(E, n_hits, S)
@@ -270,13 +296,8 @@ def run_ours(args, cfg, cid):
     del dx, dy, doff
 
     # max over ranks (device time), whole-job aggregate
-    t_ms = torch.tensor([ms_total, e2e["seconds"] if e2e else 0.0], dtype=torch.float64, device=dev)
-    tot = torch.tensor([float(E), float(n_hits)], dtype=torch.float64, device=dev)
-    if dist is not None:
-        dist.all_reduce(t_ms, op=dist.ReduceOp.MAX)
-        dist.all_reduce(tot, op=dist.ReduceOp.SUM)
-    ms_total_max, e2e_s_max = float(t_ms[0]), float(t_ms[1])
-    events_all, hits_all = float(tot[0]), float(tot[1])
+    (ms_total_max, e2e_s_max), (events_all, hits_all) = reduce_over_ranks(
+        dist, dev, [ms_total, e2e["seconds"] if e2e else 0.0], [E, n_hits])
     if dist is not None:
         dist.barrier()
         dist.destroy_process_group()
@@ -284,7 +305,7 @@ def run_ours(args, cfg, cid):
         return
 
     ms_per_step = ms_total_max / args.steps
-    value = events_all * args.steps / (ms_total_max * 1e-3)
+    value = whole_job_rate(events_all, args.steps, ms_total_max * 1e-3)
     peak, peak_src = measured_peaks()
 
     # ---- roofline of the dominant kernel: algorithmic bytes of the events it processes / its mean launch time
@@ -320,7 +341,7 @@ def run_ours(args, cfg, cid):
         "clocks": clocks, "generation_s": t_gen,
     }
     if e2e:
-        e2e_value = events_all * e2e["steps"] / e2e_s_max
+        e2e_value = whole_job_rate(events_all, e2e["steps"], e2e_s_max)
         out["e2e"] = {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": e2e["h2d_bytes"],
                       "d2h_bytes_per_step": e2e["d2h_bytes"], "steps": e2e["steps"], "slots": 2,
                       "ms_per_step": 1e3 * e2e_s_max / e2e["steps"], "h2d_gbs": e2e["h2d_bytes"] * e2e["steps"] / e2e_s_max / 1e9,
