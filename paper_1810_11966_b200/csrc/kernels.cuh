@@ -401,12 +401,13 @@ struct TeamSmem {
   uint32_t occ[2][128];                       // fine occupancy bitmaps of layers 0 and 2: row fx = 2 words, bit fy
   uint32_t J[128];                            // dilate(occ[0]) & dilate(occ[1])
   uint16_t next[2][CAP];                      // chain links (index + 1; 0 = end)
-  uint16_t surv[CAP];                         // middle hits that passed the bitmap filter
+  uint16_t surv[CAP + 32 * W];                // middle hits that passed the bitmap filter, one part per warp
+  uint32_t wcnt[W];                           // survivors in each part
   int32_t ux[2][LISTCAP], uy[2][LISTCAP];     // middle hits with triplets of the previous / current station
   uint32_t uc[2][LISTCAP];                    // their multiplicities, then saturated chain counts c_s[u]
   uint32_t off[kMaxLayers + 1];
   unsigned long long acc[2];                  // triplets of the station (parity-buffered with the two below)
-  uint32_t nsurv[2], ucount[2];
+  uint32_t ucount[2];
   uint32_t li[3];                             // ring of fetched work indices
   alignas(8) uint64_t bar;                    // completion of the station's bulk copies
 };
@@ -511,7 +512,6 @@ __global__ void __launch_bounds__(32 * W, MINB)
     sm.li[0] = atomicAdd(&ctrl->work[CLS], 1u);
     sm.li[1] = atomicAdd(&ctrl->work[CLS], 1u);
     sm.acc[0] = sm.acc[1] = 0;
-    sm.nsurv[0] = sm.nsurv[1] = 0;
     sm.ucount[0] = sm.ucount[1] = 0;
     mbar_init(&sm.bar, 1);
     fence_mbar_init();
@@ -612,6 +612,9 @@ __global__ void __launch_bounds__(32 * W, MINB)
         team_sync<W>();
         // ---- C (a6): middle hits whose fine cell is in J, compacted with ballot/popc
         const uint32_t a_J = smem_u32(sm.J);
+        constexpr uint32_t kWReg = CAP / W + 32;                  // survivors a warp can meet
+        const uint32_t a_ws = smem_u32(sm.surv) + 2u * warp * kWReg;  // this warp's part of the list (no atomics)
+        uint32_t nws = 0;
         for (uint32_t base = vwarp * 32; base < n1; base += T) {
           const uint32_t i1 = base + lane;
           bool keep = false;
@@ -622,17 +625,16 @@ __global__ void __launch_bounds__(32 * W, MINB)
             keep = (lds_u32(a_J + 4u * ((fx << 1) | (fy >> 5))) >> (fy & 31)) & 1u;
           }
           const uint32_t km = __ballot_sync(FULL, keep);
-          if (km) {
-            const int leader = __ffs(km) - 1;
-            uint32_t pos = 0;
-            if ((int)lane == leader) pos = atoms_add(&sm.nsurv[sp], (uint32_t)__popc(km));
-            pos = __shfl_sync(FULL, pos, leader);
-            if (keep) sm.surv[pos + __popc(km & lanemask_lt())] = (uint16_t)i1;
-          }
+          if (keep) sts_u16(a_ws + 2u * (nws + __popc(km & lanemask_lt())), i1);
+          nws += __popc(km);
         }
+        if (lane == 0) sm.wcnt[warp] = nws;
         team_sync<W>();
         // ---- D (a5): one lane per surviving middle hit
-        const uint32_t nsv = sm.nsurv[sp];
+        // the team's survivors, numbered through the warps' parts: number k lies in part w at k - first[w]
+        uint32_t nsv = 0, wfirst[W];
+#pragma unroll
+        for (int w = 0; w < W; ++w) { wfirst[w] = nsv; nsv += sm.wcnt[w]; }
         unsigned long long trip = 0;
         // hit with chain link cu (= index + 1) of layer 0 / 2: x at a_l + 4*cu, y kDY further; its link at a_n + 2*cu
         const uint32_t a_l0 = a_sx + 4u * o0 - 4u, a_l2 = a_sx + 4u * o2 - 4u;
@@ -643,7 +645,11 @@ __global__ void __launch_bounds__(32 * W, MINB)
           uint32_t lox = 0, hix = 0, loy = 0, hiy = 0;
           unsigned long long hq = 0;  // chain heads still to walk (16 bits each)
           if (act) {
-            const uint32_t a1 = a_sx + 4u * (o1 + sm.surv[cb + lane]);
+            const uint32_t k = cb + lane;
+            uint32_t ks = k;  // index in sm.surv
+#pragma unroll
+            for (int w = 1; w < W; ++w) if (k >= wfirst[w]) ks = k - wfirst[w] + w * kWReg;
+            const uint32_t a1 = a_sx + 4u * (o1 + sm.surv[ks]);
             x1 = lds_s32(a1);
             y1 = lds_s32<kDY>(a1);
             const int kx = __mulhi(x1, c.M1), ky = __mulhi(y1, c.M1);
@@ -730,7 +736,6 @@ __global__ void __launch_bounds__(32 * W, MINB)
       if (tid == 0) {
         n_triplets[(size_t)e * S + s] = sat32(sm.acc[sp]);
         sm.acc[sp ^ 1u] = 0;
-        sm.nsurv[sp ^ 1u] = 0;
         sm.ucount[sp ^ 1u] = 0;
         if (s + 1 < S && searchable(s + 1)) issue_stage(s + 1);
       }
