@@ -266,8 +266,12 @@ int launch_selection(cbm_trigger* h, const Scratch& scr, const int32_t* d_x, con
   if (n_events == 0) return 0;
   if (prof) CBM_CUDA(h, cudaEventRecord(prof->k[0], st));
   const uint32_t n_tiles = (n_events + kTileEvents - 1) / kTileEvents;
-  tile_kernel<<<n_tiles, kTileEvents * p.S, 0, st>>>(p, d_x, d_y, d_off, n_events, (uint32_t)n_hits, d_nt, d_nc, d_ac,
-                                                     scr.d_ctrl, scr.d_list[kClsM], scr.d_list[kClsH], scr.d_list[kClsG]);
+  if (p.S <= 4)  // tables sized for 4 stations: more resident CTAs
+    tile_kernel<4><<<n_tiles, kTileEvents * p.S, 0, st>>>(p, d_x, d_y, d_off, n_events, (uint32_t)n_hits, d_nt, d_nc, d_ac,
+                                                          scr.d_ctrl, scr.d_list[kClsM], scr.d_list[kClsH], scr.d_list[kClsG]);
+  else
+    tile_kernel<kMaxStations><<<n_tiles, kTileEvents * p.S, 0, st>>>(p, d_x, d_y, d_off, n_events, (uint32_t)n_hits, d_nt, d_nc, d_ac,
+                                                                     scr.d_ctrl, scr.d_list[kClsM], scr.d_list[kClsH], scr.d_list[kClsG]);
   if (prof) CBM_CUDA(h, cudaEventRecord(prof->k[1], st));
   TEAM_KERNEL_M<<<h->grid[kClsM], 32 * kWM, 0, st>>>(
       p, d_x, d_y, d_off, d_nt, d_nc, d_ac, scr.d_ctrl, scr.d_list[kClsM], scr.d_spill[kClsM]);
@@ -361,6 +365,8 @@ int cbm_trigger_create(const cbm_trigger_config_t* cfg, cbm_trigger_t** out) {
   if (prop.major < 10) { fail(h, CBM_ERR_CUDA, "device is sm_%d%d; this library holds sm_100a code only", prop.major, prop.minor); return bail(CBM_ERR_CUDA); }
   h->n_sm = prop.multiProcessorCount;
   static_assert(sizeof(SmemM) <= 48 * 1024 && sizeof(SmemH) <= 48 * 1024, "static shared memory limit");
+  CREATE_CUDA(cudaFuncSetAttribute(tile_kernel<4>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
+  CREATE_CUDA(cudaFuncSetAttribute(tile_kernel<kMaxStations>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
   CREATE_TRY(occupancy_grid(h, TEAM_KERNEL_M, 32 * kWM, 0, &h->grid[kClsM]));
   CREATE_TRY(occupancy_grid(h, TEAM_KERNEL_H, 32 * kWH, 0, &h->grid[kClsH]));
   CREATE_TRY(occupancy_grid(h, TEAM_KERNEL_G, 32 * kWG, sizeof(SmemG), &h->grid[kClsG]));

@@ -101,17 +101,18 @@ struct TileStation {  // constants of one station, read from shared memory (lane
   int32_t z0, z1, z2, pad;
   int64_t T01, T02, T12;
 };
+template <int MS>  // MS: stations the tables are sized for (4 or 8)
 struct TileSmem {
   alignas(16) int32_t sx[kTileHitCap];
   alignas(16) int32_t sy[kTileHitCap];
-  alignas(16) TileStation sc[kMaxStations];
-  uint32_t off[kTileEvents * kMaxLayers + 1];
+  alignas(16) TileStation sc[MS];
+  uint32_t off[kTileEvents * 3 * MS + 1];
   uint32_t ev_max[kTileEvents];
   uint32_t ev_dst[kTileEvents];
-  uint32_t st_cnt[kTileEvents * kMaxStations];  // triplets of (event el, station s) at [el*S + s]
-  uint32_t pre[kTileEvents * kMaxStations];     // first search unit of (station, event) thread t
-  alignas(8) uint2 desc[kTileEvents * kMaxStations];  // its layer boundaries in sx/sy: (b0 | b1<<16, b2 | b3<<16)
-  uint32_t wsum[kMaxStations];
+  uint32_t st_cnt[kTileEvents * MS];            // triplets of (event el, station s) at [el*S + s]
+  uint32_t pre[kTileEvents * MS];               // first search unit of (station, event) thread t
+  alignas(8) uint2 desc[kTileEvents * MS];      // its layer boundaries in sx/sy: (b0 | b1<<16, b2 | b3<<16)
+  uint32_t wsum[MS];
   uint32_t f_key[kTileFound];                   // found (h0,h1) pairs with triplets: owner thread << 16 | index of h1
   uint32_t f_t[kTileFound];                     // number of h2 completing the pair
   uint32_t f_c[kTileFound];                     // chain count of the entry (a7)
@@ -120,12 +121,13 @@ struct TileSmem {
   alignas(8) uint64_t bar;
 };
 
-__global__ void __launch_bounds__(kTileEvents* kMaxStations)
+template <int MS>
+__global__ void __launch_bounds__(kTileEvents* MS)
     tile_kernel(const __grid_constant__ Params p, const int32_t* __restrict__ x, const int32_t* __restrict__ y,
                 const uint32_t* __restrict__ off, uint32_t n_events, uint32_t n_hits, uint32_t* __restrict__ n_triplets,
                 uint32_t* __restrict__ n_candidates, uint8_t* __restrict__ accept, Ctrl* __restrict__ ctrl,
                 uint32_t* __restrict__ list_M, uint32_t* __restrict__ list_H, uint32_t* __restrict__ list_G) {
-  __shared__ TileSmem sm;
+  __shared__ TileSmem<MS> sm;
   constexpr uint32_t FULL = 0xFFFFFFFFu;
   const uint32_t tid = threadIdx.x, nthr = blockDim.x;
   const uint32_t S = p.S, L = p.L;
@@ -173,7 +175,16 @@ __global__ void __launch_bounds__(kTileEvents* kMaxStations)
     const uint32_t ob = in ? sm.off[lane * L] : 0u, oe = in ? sm.off[(lane + 1) * L] : 0u;
     const bool invalid = in && mx == 0xFFFFFFFFu;
     const uint32_t tot = oe - ob;
-    const bool tiny = in && !invalid && p.tiny_max_total != 0 && mx <= p.tiny_max_layer && tot <= p.tiny_max_total;
+    bool tiny = in && !invalid && p.tiny_max_total != 0 && mx <= p.tiny_max_layer && tot <= p.tiny_max_total;
+    {  // the tile's staging buffer: tiny events are admitted in order while they fit
+      uint32_t need = tiny ? tot + kTinySlack : 0u;
+#pragma unroll
+      for (int d = 1; d < 32; d <<= 1) {
+        const uint32_t v = __shfl_up_sync(FULL, need, d);
+        if (lane >= (uint32_t)d) need += v;
+      }
+      tiny = tiny && need <= kTileHitCap;
+    }
     const uint32_t tmask = __ballot_sync(FULL, tiny);
     // my run = maximal block of consecutive tiny events around me; runs are contiguous in x[] / y[]
     const uint32_t nz_below = (~tmask) & ((1u << lane) - 1u);
@@ -191,7 +202,7 @@ __global__ void __launch_bounds__(kTileEvents* kMaxStations)
       if (lane >= (uint32_t)d) incl += v;
     }
     const uint32_t excl = incl - run_len;
-    const uint32_t total = __shfl_sync(FULL, incl, 31);  // <= kTileHitCap by construction (params.h)
+    const uint32_t total = __shfl_sync(FULL, incl, 31);  // <= kTileHitCap: every run is shorter than its events + slack
     const uint32_t run_dst = __shfl_sync(FULL, excl, rs);
     sm.ev_dst[lane] = tiny ? run_dst + (ob - run_src) : kNotTiny;
     if (lane == 0) mbar_arrive_expect_tx(&sm.bar, total * 8u);
@@ -270,7 +281,7 @@ __global__ void __launch_bounds__(kTileEvents* kMaxStations)
     const int32_t z0 = k.z0, z1 = k.z1, nz0 = -z0;
     const int64_t T01 = k.T01;
     const uint64_t T01x2 = 2 * (uint64_t)T01;
-    constexpr int kDY = (int)(offsetof(TileSmem, sy) - offsetof(TileSmem, sx));
+    constexpr int kDY = (int)(offsetof(TileSmem<MS>, sy) - offsetof(TileSmem<MS>, sx));
     const uint32_t ax = smem_u32(sm.sx);
     const int32_t x0 = lds_s32(ax + 4 * (b0 + i0)), y0 = lds_s32<kDY>(ax + 4 * (b0 + i0));
     // |x0*z1 - x1*z0| <= T01  <=>  (uint64)(x1*(-z0) + (x0*z1 + T01)) <= 2*T01

@@ -54,7 +54,11 @@ static_assert(sizeof(Ctrl) == 64, "Ctrl is copied as one 64-byte record");
 // tile kernel geometry
 constexpr int kTileEvents = 32;              // events per CTA of the tile kernel = lanes of the planning warp
 constexpr uint32_t kTinyMaxTotal = 96;       // a tiny event holds at most this many hits ...
-constexpr uint32_t kTileHitCap = kTileEvents * kTinyMaxTotal + 32;  // ... so a tile never overflows this (see tile_kernel)
+constexpr uint32_t kTinySlack = 6;           // ... plus at most 3 + 3 hits of 16-byte alignment around its run
+// Hits a tile stages in shared memory.  Tiny events are admitted in order while their sizes (+ slack) fit; the
+// few that do not (a tile of 32 events near the 96-hit limit) go to class M.  2304 = 32 x (66 + 6): the load-
+// imbalance workload's minimum-bias events hold 60 +- 8 hits.
+constexpr uint32_t kTileHitCap = 2304;
 constexpr uint32_t kTinyMaxLayerLimit = 32;
 constexpr int kTileFound = 64;               // (h0,h1) pairs with triplets a tile links itself; more: class M
 
