@@ -288,31 +288,40 @@ __global__ void __launch_bounds__(kTileEvents* MS)
     const int64_t Px = (int64_t)x0 * z1 + T01, Py = (int64_t)y0 * z1 + T01;
     uint32_t cnt = 0;
     const uint32_t a_end = ax + 4 * b2;
-    for (uint32_t a1 = ax + 4 * b1; a1 != a_end; a1 += 4) {
-      const int32_t x1 = lds_s32(a1);
-      if ((uint64_t)((int64_t)x1 * nz0 + Px) <= T01x2) {
-        const int32_t y1 = lds_s32<kDY>(a1);
-        if ((uint64_t)((int64_t)y1 * nz0 + Py) <= T01x2) {
-          const int32_t z2 = k.z2;
-          const int64_t T02 = k.T02, T12 = k.T12;
-          const int64_t Qx0 = (int64_t)x0 * z2 + T02, Qy0 = (int64_t)y0 * z2 + T02;
-          const int64_t Qx1 = (int64_t)x1 * z2 + T12, Qy1 = (int64_t)y1 * z2 + T12;
-          uint32_t t = 0;
-          for (uint32_t i2 = b2; i2 < b3; ++i2) {
-            const int32_t x2 = sm.sx[i2], y2 = sm.sy[i2];
-            const bool ok = win(Qx0, x2, z0, 2 * (uint64_t)T02) & win(Qy0, y2, z0, 2 * (uint64_t)T02) &
-                            win(Qx1, x2, z1, 2 * (uint64_t)T12) & win(Qy1, y2, z1, 2 * (uint64_t)T12);
-            t += ok ? 1u : 0u;
-          }
-          if (t) {
-            cnt += t;
-            const uint32_t slot = atomicAdd(&sm.nfound, 1u);
-            if (slot < (uint32_t)kTileFound) {
-              sm.f_key[slot] = (ow << 16) | ((a1 - ax) >> 2);
-              sm.f_t[slot] = t;
-            }
+    // the rare continuation of a pair that passed the x test: y test, then the h2 loop
+    auto pair_passed_x = [&](uint32_t a1, int32_t x1) {
+      const int32_t y1 = lds_s32<kDY>(a1);
+      if ((uint64_t)((int64_t)y1 * nz0 + Py) <= T01x2) {
+        const int32_t z2 = k.z2;
+        const int64_t T02 = k.T02, T12 = k.T12;
+        const int64_t Qx0 = (int64_t)x0 * z2 + T02, Qy0 = (int64_t)y0 * z2 + T02;
+        const int64_t Qx1 = (int64_t)x1 * z2 + T12, Qy1 = (int64_t)y1 * z2 + T12;
+        uint32_t t = 0;
+        for (uint32_t i2 = b2; i2 < b3; ++i2) {
+          const int32_t x2 = sm.sx[i2], y2 = sm.sy[i2];
+          const bool ok = win(Qx0, x2, z0, 2 * (uint64_t)T02) & win(Qy0, y2, z0, 2 * (uint64_t)T02) &
+                          win(Qx1, x2, z1, 2 * (uint64_t)T12) & win(Qy1, y2, z1, 2 * (uint64_t)T12);
+          t += ok ? 1u : 0u;
+        }
+        if (t) {
+          cnt += t;
+          const uint32_t slot = atomicAdd(&sm.nfound, 1u);
+          if (slot < (uint32_t)kTileFound) {
+            sm.f_key[slot] = (ow << 16) | ((a1 - ax) >> 2);
+            sm.f_t[slot] = t;
           }
         }
+      }
+    };
+    // two pairs per trip: two independent load/test chains, half the loop overhead (the second load of an odd
+    // last trip reads the next layer's first hit; its result is masked)
+    for (uint32_t a1 = ax + 4 * b1; a1 < a_end; a1 += 8) {
+      const int32_t xa = lds_s32(a1), xb = lds_s32<4>(a1);
+      const bool pa = (uint64_t)((int64_t)xa * nz0 + Px) <= T01x2;
+      const bool pb = ((uint64_t)((int64_t)xb * nz0 + Px) <= T01x2) & (a1 + 4 < a_end);
+      if (pa | pb) {
+        if (pa) pair_passed_x(a1, xa);
+        if (pb) pair_passed_x(a1 + 4, xb);
       }
     }
     if (cnt) atomicAdd(&sm.st_cnt[(ow & 31u) * S + (ow >> 5)], cnt);
