@@ -43,7 +43,7 @@ struct Scratch {
 };
 
 struct ProfEvents {
-  cudaEvent_t k[CBM_TRIGGER_N_KERNELS + 1] = {};
+  cudaEvent_t k[2 * CBM_TRIGGER_N_KERNELS] = {};  // start, end of every kernel
   cudaEvent_t h2d[2] = {}, d2h[2] = {};
   bool valid = false;
 };
@@ -82,6 +82,8 @@ struct cbm_trigger {
   uint32_t dev_n_events = 0;
   uint64_t dev_n_hits = 0;
   cudaStream_t st_h2d = nullptr, st_run = nullptr, st_d2h = nullptr;
+  cudaStream_t st_side[2] = {nullptr, nullptr};  // classes M and G run beside class H (after the tile kernel)
+  cudaEvent_t ev_fork = nullptr, ev_join[2] = {nullptr, nullptr};
   std::string err;
 };
 
@@ -273,15 +275,27 @@ int launch_selection(cbm_trigger* h, const Scratch& scr, const int32_t* d_x, con
     tile_kernel<kMaxStations><<<n_tiles, kTileEvents * p.S, 0, st>>>(p, d_x, d_y, d_off, n_events, (uint32_t)n_hits, d_nt, d_nc, d_ac,
                                                                      scr.d_ctrl, scr.d_list[kClsM], scr.d_list[kClsH], scr.d_list[kClsG]);
   if (prof) CBM_CUDA(h, cudaEventRecord(prof->k[1], st));
-  TEAM_KERNEL_M<<<h->grid[kClsM], 32 * kWM, 0, st>>>(
+  // The three class kernels are independent (disjoint events): M and G on side streams, H on the caller's.
+  // M and G are launched first: most of their persistent CTAs find an empty list and leave at once.
+  CBM_CUDA(h, cudaEventRecord(h->ev_fork, st));
+  CBM_CUDA(h, cudaStreamWaitEvent(h->st_side[0], h->ev_fork, 0));
+  CBM_CUDA(h, cudaStreamWaitEvent(h->st_side[1], h->ev_fork, 0));
+  if (prof) CBM_CUDA(h, cudaEventRecord(prof->k[2], h->st_side[0]));
+  TEAM_KERNEL_M<<<h->grid[kClsM], 32 * kWM, 0, h->st_side[0]>>>(
       p, d_x, d_y, d_off, d_nt, d_nc, d_ac, scr.d_ctrl, scr.d_list[kClsM], scr.d_spill[kClsM]);
-  if (prof) CBM_CUDA(h, cudaEventRecord(prof->k[2], st));
+  if (prof) CBM_CUDA(h, cudaEventRecord(prof->k[3], h->st_side[0]));
+  CBM_CUDA(h, cudaEventRecord(h->ev_join[0], h->st_side[0]));
+  if (prof) CBM_CUDA(h, cudaEventRecord(prof->k[6], h->st_side[1]));
+  TEAM_KERNEL_G<<<h->grid[kClsG], 32 * kWG, sizeof(SmemG), h->st_side[1]>>>(
+      p, d_x, d_y, d_off, d_nt, d_nc, d_ac, scr.d_ctrl, scr.d_list[kClsG], scr.d_spill[kClsG]);
+  if (prof) CBM_CUDA(h, cudaEventRecord(prof->k[7], h->st_side[1]));
+  CBM_CUDA(h, cudaEventRecord(h->ev_join[1], h->st_side[1]));
+  if (prof) CBM_CUDA(h, cudaEventRecord(prof->k[4], st));
   TEAM_KERNEL_H<<<h->grid[kClsH], 32 * kWH, 0, st>>>(
       p, d_x, d_y, d_off, d_nt, d_nc, d_ac, scr.d_ctrl, scr.d_list[kClsH], scr.d_spill[kClsH]);
-  if (prof) CBM_CUDA(h, cudaEventRecord(prof->k[3], st));
-  TEAM_KERNEL_G<<<h->grid[kClsG], 32 * kWG, sizeof(SmemG), st>>>(
-      p, d_x, d_y, d_off, d_nt, d_nc, d_ac, scr.d_ctrl, scr.d_list[kClsG], scr.d_spill[kClsG]);
-  if (prof) { CBM_CUDA(h, cudaEventRecord(prof->k[4], st)); prof->valid = true; }
+  if (prof) { CBM_CUDA(h, cudaEventRecord(prof->k[5], st)); prof->valid = true; }
+  CBM_CUDA(h, cudaStreamWaitEvent(st, h->ev_join[0], 0));
+  CBM_CUDA(h, cudaStreamWaitEvent(st, h->ev_join[1], 0));
   CBM_CUDA(h, cudaGetLastError());
   return 4;
 }
@@ -303,7 +317,7 @@ void fill_prof(cbm_trigger_stats_t& st, ProfEvents& pe, bool copies) {
   if (!pe.valid) return;
   for (int k = 0; k < CBM_TRIGGER_N_KERNELS; ++k) {
     float ms = 0;
-    if (cudaEventElapsedTime(&ms, pe.k[k], pe.k[k + 1]) == cudaSuccess) st.kernel_ms[k] = ms;
+    if (cudaEventElapsedTime(&ms, pe.k[2 * k], pe.k[2 * k + 1]) == cudaSuccess) st.kernel_ms[k] = ms;
   }
   if (copies) {
     float ms = 0;
@@ -373,6 +387,9 @@ int cbm_trigger_create(const cbm_trigger_config_t* cfg, cbm_trigger_t** out) {
   CREATE_CUDA(cudaStreamCreateWithFlags(&h->st_h2d, cudaStreamNonBlocking));
   CREATE_CUDA(cudaStreamCreateWithFlags(&h->st_run, cudaStreamNonBlocking));
   CREATE_CUDA(cudaStreamCreateWithFlags(&h->st_d2h, cudaStreamNonBlocking));
+  for (auto& sd : h->st_side) CREATE_CUDA(cudaStreamCreateWithFlags(&sd, cudaStreamNonBlocking));
+  CREATE_CUDA(cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming));
+  for (auto& ej : h->ev_join) CREATE_CUDA(cudaEventCreateWithFlags(&ej, cudaEventDisableTiming));
   CREATE_TRY(alloc_scratch(h, h->dev_scr));
   CREATE_CUDA(cudaHostAlloc(&h->h_dev_ctrl, sizeof(Ctrl), cudaHostAllocDefault));
   if (cfg->flags & CBM_FLAG_PROFILE)
@@ -399,6 +416,9 @@ void cbm_trigger_destroy(cbm_trigger_t* h) {
   if (h->st_h2d) cudaStreamDestroy(h->st_h2d);
   if (h->st_run) cudaStreamDestroy(h->st_run);
   if (h->st_d2h) cudaStreamDestroy(h->st_d2h);
+  for (auto& sd : h->st_side) if (sd) cudaStreamDestroy(sd);
+  if (h->ev_fork) cudaEventDestroy(h->ev_fork);
+  for (auto& ej : h->ev_join) if (ej) cudaEventDestroy(ej);
   delete h;
 }
 
@@ -561,7 +581,7 @@ int cbm_trigger_device_kernel_times(cbm_trigger_t* h, void* stream, uint32_t n_l
     ProfEvents& pe = h->dev_prof[(h->dev_prof_head - n + i) % CBM_TRIGGER_PROFILE_RING];
     for (int k = 0; k < CBM_TRIGGER_N_KERNELS; ++k) {
       float ms = 0;
-      if (pe.valid) CBM_CUDA(h, cudaEventElapsedTime(&ms, pe.k[k], pe.k[k + 1]));
+      if (pe.valid) CBM_CUDA(h, cudaEventElapsedTime(&ms, pe.k[2 * k], pe.k[2 * k + 1]));
       kernel_ms[i * CBM_TRIGGER_N_KERNELS + k] = ms;
     }
   }
