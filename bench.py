@@ -35,7 +35,7 @@ CBM_INTERACTION_RATE_HZ = 1.0e7
 def parse_args():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json configs index (0..3; 4 = streaming of config-2 chunks)")
@@ -74,7 +74,7 @@ class ClockSampler:
         try:
             self.proc = subprocess.Popen(
                 ["nvidia-smi", f"--id={self.device_index}", f"--query-gpu={self.QUERY}", "--format=csv,noheader,nounits",
-                 "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+                 "-lms", "20"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
         except Exception:
             self.proc = None
             return
@@ -360,7 +360,10 @@ def run_ours(args, cfg, cid):
 
 # per-launch DRAM traffic (dram__bytes_read.sum + dram__bytes_write.sum) of one `ncu --set full` capture,
 # copied by hand from profiles/ (see the .md there); None until a capture exists for that kernel.
-NCU_TRAFFIC_BYTES = {}
+NCU_TRAFFIC_BYTES = {
+    ("cfg3_imbalance", "team_kernel_H"): 1_754_425_000 + 8_558_848,   # profiles/r1_team_kernel_H.md
+    ("cfg3_imbalance", "tile_kernel"): 519_462_144 + 20_825_856,      # profiles/r1_tile_kernel.md
+}
 
 
 def run_e2e(args, cfg, cid, batch, K, W, local_rank, rank, barrier):
@@ -369,7 +372,7 @@ def run_e2e(args, cfg, cid, batch, K, W, local_rank, rank, barrier):
     overlaps the kernels and the D2H of batch i.  Wall clock between device synchronisations."""
     import torch
     E, S, L = batch.n_events, cfg.n_stations, cfg.n_layers
-    steps = args.e2e_steps or min(args.steps, 10)
+    steps = args.e2e_steps or min(max(args.steps, 2), 10)
     batches = [batch]
     if cfg.chunk_events:  # config 4: distinct chunks in the two slots
         batches.append(W.generate(cfg, n_events=E, first_event=(rank + 1) * E + 7 * E))
