@@ -129,6 +129,21 @@ int cbm_trigger_run(cbm_trigger_t* h, uint32_t slot);
 int cbm_trigger_fetch_results(cbm_trigger_t* h, uint32_t slot, uint32_t* n_triplets, uint32_t* n_candidates,
                               uint8_t* accept);
 
+/* The list of selected events ("the list of selected events is transferred back to the host"):
+ * the ids of the events of the slot's last run with accept != 0, in ascending order (so the list is unique),
+ * built on the device by an order-preserving compaction of accept[] as part of `run`.  Blocks until the run's
+ * results are on the host.  event_ids: HOST, room for `capacity` uint32; n_selected: HOST, always written.
+ * Returns CBM_ERR_CAPACITY (and writes only *n_selected) if more than `capacity` events were selected,
+ * CBM_ERR_STATE without a preceding run.  May be called before or after fetch_results, until the next upload. */
+int cbm_trigger_fetch_selected(cbm_trigger_t* h, uint32_t slot, uint32_t* event_ids, uint32_t capacity,
+                               uint32_t* n_selected);
+
+/* The same compaction on caller-owned DEVICE arrays on the caller's stream (see cbm_trigger_run_device):
+ * d_accept[n_events] uint8 in; d_event_ids (room for n_events uint32) and d_n_selected (one uint32) out.
+ * Asynchronous; uses the handle's scheduler scratch, so calls on one handle must be stream-ordered. */
+int cbm_trigger_select_device(cbm_trigger_t* h, uint32_t n_events, const uint8_t* d_accept, uint32_t* d_event_ids,
+                              uint32_t* d_n_selected, void* stream);
+
 /* Device-resident entry point (PyTorch or any other owner of device memory and streams supplies both):
  * runs a3-a8 on caller-owned DEVICE arrays on the caller's stream (`stream` is a cudaStream_t passed as void*;
  * NULL = the legacy default stream).  d_x, d_y: n_hits int32 each, 16-byte aligned, readable up to the next

@@ -130,3 +130,13 @@ def run_slope_sorted(geo: Geometry, x, y, off, e_begin=0, e_end=None):
     if rc != 0:
         raise RuntimeError(f"cbm_slope_sorted_run failed: {rc}")
     return nt, nc, ac, int(ne.value)
+
+
+def selected(accept):
+    """The list of selected events ("the list of selected events is transferred back"): the ids of
+    the events with accept != 0 in ascending order.  Written out as the plain loop it is."""
+    ids = []
+    for e, a in enumerate(np.asarray(accept).ravel().tolist()):
+        if a:
+            ids.append(e)
+    return np.asarray(ids, dtype=np.uint32)

@@ -23,6 +23,7 @@ EXPORTS = (
     "cbm_trigger_create", "cbm_trigger_destroy", "cbm_trigger_host_buffers", "cbm_trigger_upload_events",
     "cbm_trigger_run", "cbm_trigger_fetch_results", "cbm_trigger_run_device", "cbm_trigger_device_status",
     "cbm_trigger_get_stats", "cbm_trigger_last_error", "cbm_trigger_version", "cbm_trigger_device_kernel_times",
+    "cbm_trigger_fetch_selected", "cbm_trigger_select_device",
 )
 PROFILE_RING = 32
 # scheduler classes (csrc/cbm_trigger.cu, csrc/params.h), restated for bookkeeping in bench.py only
@@ -105,6 +106,10 @@ def load_library():
         lib.cbm_trigger_device_status.argtypes = [vp, vp, ctypes.POINTER(Stats)]
         lib.cbm_trigger_device_kernel_times.restype = i32
         lib.cbm_trigger_device_kernel_times.argtypes = [vp, vp, u32, vp]
+        lib.cbm_trigger_fetch_selected.restype = i32
+        lib.cbm_trigger_fetch_selected.argtypes = [vp, u32, vp, u32, ctypes.POINTER(u32)]
+        lib.cbm_trigger_select_device.restype = i32
+        lib.cbm_trigger_select_device.argtypes = [vp, u32, vp, vp, vp, vp]
         lib.cbm_trigger_get_stats.restype = i32
         lib.cbm_trigger_get_stats.argtypes = [vp, u32, ctypes.POINTER(Stats)]
         lib.cbm_trigger_last_error.restype = ctypes.c_char_p
@@ -193,6 +198,20 @@ def cbm_trigger_fetch_results(handle, slot, n_triplets, n_candidates, accept):
     return rc
 
 
+def cbm_trigger_fetch_selected(handle, slot, event_ids):
+    """Fills event_ids (uint32 numpy array = the capacity); returns the number of selected events."""
+    n = ctypes.c_uint32(0)
+    rc = load_library().cbm_trigger_fetch_selected(handle, slot, _host_ptr(event_ids, np.uint32) if event_ids.size else None,
+                                                   event_ids.size, ctypes.byref(n))
+    _check(rc, handle)
+    return int(n.value)
+
+
+def cbm_trigger_select_device(handle, n_events, d_accept, d_event_ids, d_n_selected, stream=0):
+    """d_* are raw device addresses (ints); stream is a cudaStream_t as int."""
+    _check(load_library().cbm_trigger_select_device(handle, n_events, d_accept, d_event_ids, d_n_selected, stream), handle)
+
+
 def cbm_trigger_get_stats(handle, slot) -> Stats:
     st = Stats()
     _check(load_library().cbm_trigger_get_stats(handle, slot, ctypes.byref(st)), handle)
@@ -273,6 +292,17 @@ class Trigger:
 
     def stats(self, slot) -> Stats:
         return cbm_trigger_get_stats(self.handle, slot)
+
+    def fetch_selected(self, slot, capacity=None):
+        """Ascending ids of the accepted events of the slot's last run."""
+        ids = np.empty(self.cfg.max_events if capacity is None else capacity, dtype=np.uint32)
+        n = cbm_trigger_fetch_selected(self.handle, slot, ids)
+        return ids[:n].copy()
+
+    def select_device(self, n_events, d_ac, d_ids, d_n, stream=None):
+        import torch
+        st = torch.cuda.current_stream().cuda_stream if stream is None else stream
+        cbm_trigger_select_device(self.handle, n_events, d_ac.data_ptr(), d_ids.data_ptr(), d_n.data_ptr(), st)
 
     def select(self, x, y, off, slot=0):
         """upload + run + fetch of one host batch (numpy arrays)."""

@@ -16,6 +16,7 @@
 
 #include "../../include/cbm_trigger.h"
 #include "kernels.cuh"
+#include "select.cuh"
 
 namespace {
 
@@ -40,6 +41,7 @@ struct Scratch {
   Ctrl* d_ctrl = nullptr;
   uint32_t* d_list[kNumTeamClasses] = {nullptr, nullptr, nullptr};
   uint32_t* d_spill[kNumTeamClasses] = {nullptr, nullptr, nullptr};  // per CTA: middle-hit lists beyond shared memory
+  uint32_t* d_selcnt = nullptr;  // accepted events per block of kSelEvents events (select.cuh)
 };
 
 struct ProfEvents {
@@ -55,6 +57,9 @@ struct Slot {
   uint32_t* d_off = nullptr;
   uint32_t *d_nt = nullptr, *d_nc = nullptr;
   uint8_t* d_ac = nullptr;
+  uint32_t *d_sel = nullptr, *d_nsel = nullptr;  // ascending ids of the accepted events, their number
+  uint32_t* h_nsel = nullptr;
+  bool sel_valid = false;
   uint32_t *h_nt = nullptr, *h_nc = nullptr;
   uint8_t* h_ac = nullptr;
   Ctrl* h_ctrl = nullptr;
@@ -191,6 +196,7 @@ int build_params(const cbm_trigger_config_t& c, Params& p, std::string& why) {
 // ---------------------------------------------------------------------------------------------- allocation
 int alloc_scratch(cbm_trigger* h, Scratch& s) {
   CBM_CUDA(h, cudaMalloc(&s.d_ctrl, sizeof(Ctrl)));
+  CBM_CUDA(h, cudaMalloc(&s.d_selcnt, ((size_t)h->cfg.max_events / kSelEvents + 1) * sizeof(uint32_t)));
   const size_t cap[kNumTeamClasses] = {kCapM, kCapH, kCapG};
   for (int c = 0; c < kNumTeamClasses; ++c) {
     CBM_CUDA(h, cudaMalloc(&s.d_list[c], (size_t)h->cfg.max_events * sizeof(uint32_t)));
@@ -200,6 +206,7 @@ int alloc_scratch(cbm_trigger* h, Scratch& s) {
 }
 void free_scratch(Scratch& s) {
   cudaFree(s.d_ctrl);
+  cudaFree(s.d_selcnt);
   for (int c = 0; c < kNumTeamClasses; ++c) { cudaFree(s.d_list[c]); cudaFree(s.d_spill[c]); }
   s = Scratch();
 }
@@ -230,6 +237,9 @@ int alloc_slot(cbm_trigger* h, Slot& s) {
   CBM_CUDA(h, cudaMalloc(&s.d_nt, ne * S * 4));
   CBM_CUDA(h, cudaMalloc(&s.d_nc, ne * 4));
   CBM_CUDA(h, cudaMalloc(&s.d_ac, ne));
+  CBM_CUDA(h, cudaMalloc(&s.d_sel, ne * 4));
+  CBM_CUDA(h, cudaMalloc(&s.d_nsel, 4));
+  CBM_CUDA(h, cudaHostAlloc(&s.h_nsel, 4, cudaHostAllocDefault));
   CBM_CUDA(h, cudaHostAlloc(&s.h_nt, ne * S * 4, cudaHostAllocDefault));
   CBM_CUDA(h, cudaHostAlloc(&s.h_nc, ne * 4, cudaHostAllocDefault));
   CBM_CUDA(h, cudaHostAlloc(&s.h_ac, ne, cudaHostAllocDefault));
@@ -248,6 +258,7 @@ void free_slot(Slot& s) {
   cudaFreeHost(s.h_x); cudaFreeHost(s.h_y); cudaFreeHost(s.h_off);
   cudaFree(s.d_x); cudaFree(s.d_y); cudaFree(s.d_off);
   cudaFree(s.d_nt); cudaFree(s.d_nc); cudaFree(s.d_ac);
+  cudaFree(s.d_sel); cudaFree(s.d_nsel); cudaFreeHost(s.h_nsel);
   cudaFreeHost(s.h_nt); cudaFreeHost(s.h_nc); cudaFreeHost(s.h_ac); cudaFreeHost(s.h_ctrl);
   free_scratch(s.scr);
   free_prof(s.prof);
@@ -298,6 +309,20 @@ int launch_selection(cbm_trigger* h, const Scratch& scr, const int32_t* d_x, con
   CBM_CUDA(h, cudaStreamWaitEvent(st, h->ev_join[1], 0));
   CBM_CUDA(h, cudaGetLastError());
   return 4;
+}
+
+// The list of selected events: ascending ids of the events with accept != 0, and their number.
+int launch_compaction(cbm_trigger* h, const Scratch& scr, const uint8_t* d_ac, uint32_t n_events, uint32_t* d_sel,
+                      uint32_t* d_nsel, cudaStream_t st) {
+  if (n_events == 0) {
+    CBM_CUDA(h, cudaMemsetAsync(d_nsel, 0, sizeof(uint32_t), st));
+    return 0;
+  }
+  const uint32_t nb = (n_events + kSelEvents - 1) / kSelEvents;
+  select_count_kernel<<<nb, kSelThreads, 0, st>>>(d_ac, n_events, scr.d_selcnt);
+  select_write_kernel<<<nb, kSelThreads, 0, st>>>(d_ac, n_events, scr.d_selcnt, d_sel, d_nsel);
+  CBM_CUDA(h, cudaGetLastError());
+  return 2;
 }
 
 void fill_stats(cbm_trigger_stats_t& st, const Ctrl& c, uint32_t n_events, uint64_t n_hits, uint32_t n_launches) {
@@ -467,6 +492,7 @@ int cbm_trigger_upload_events(cbm_trigger_t* h, uint32_t slot, uint32_t n_events
   CBM_CUDA(h, cudaEventRecord(s.ev_h2d, h->st_h2d));
   s.n_events = n_events;
   s.n_hits = n_hits;
+  s.sel_valid = false;
   s.state = kUploaded;
   return CBM_OK;
 }
@@ -483,6 +509,8 @@ int cbm_trigger_run(cbm_trigger_t* h, uint32_t slot) {
   const int nl = launch_selection(h, s.scr, s.d_x, s.d_y, s.d_off, s.n_events, s.n_hits, s.d_nt, s.d_nc, s.d_ac,
                                   h->st_run, prof ? &s.prof : nullptr);
   if (nl < 0) return nl;
+  const int nl2 = launch_compaction(h, s.scr, s.d_ac, s.n_events, s.d_sel, s.d_nsel, h->st_run);
+  if (nl2 < 0) return nl2;
   CBM_CUDA(h, cudaEventRecord(s.ev_run, h->st_run));
   CBM_CUDA(h, cudaStreamWaitEvent(h->st_d2h, s.ev_run, 0));
   if (prof) CBM_CUDA(h, cudaEventRecord(s.prof.d2h[0], h->st_d2h));
@@ -493,9 +521,11 @@ int cbm_trigger_run(cbm_trigger_t* h, uint32_t slot) {
     CBM_CUDA(h, cudaMemcpyAsync(s.h_ac, s.d_ac, ne, cudaMemcpyDeviceToHost, h->st_d2h));
   }
   CBM_CUDA(h, cudaMemcpyAsync(s.h_ctrl, s.scr.d_ctrl, sizeof(Ctrl), cudaMemcpyDeviceToHost, h->st_d2h));
+  CBM_CUDA(h, cudaMemcpyAsync(s.h_nsel, s.d_nsel, sizeof(uint32_t), cudaMemcpyDeviceToHost, h->st_d2h));
   if (prof) CBM_CUDA(h, cudaEventRecord(s.prof.d2h[1], h->st_d2h));
   CBM_CUDA(h, cudaEventRecord(s.ev_d2h, h->st_d2h));
-  s.stats.n_launches = (uint32_t)nl;
+  s.stats.n_launches = (uint32_t)(nl + nl2);
+  s.sel_valid = true;
   s.state = kRunning;
   return CBM_OK;
 }
@@ -523,6 +553,36 @@ int cbm_trigger_fetch_results(cbm_trigger_t* h, uint32_t slot, uint32_t* n_tripl
     return fail(h, CBM_ERR_RANGE, "%u event(s) rejected on the device (offsets not monotone, beyond n_hits, or a layer above max_hits_per_layer); first: event %u",
                 s.stats.n_invalid, s.stats.first_invalid);
   return CBM_OK;
+}
+
+int cbm_trigger_fetch_selected(cbm_trigger_t* h, uint32_t slot, uint32_t* event_ids, uint32_t capacity,
+                               uint32_t* n_selected) {
+  int rc = check_slot(h, slot);
+  if (rc) return rc;
+  Slot& s = h->slot[slot];
+  if (!s.sel_valid) return fail(h, CBM_ERR_STATE, "slot %u: fetch_selected needs a preceding run", slot);
+  if (!n_selected) return fail(h, CBM_ERR_INVALID_ARG, "n_selected must not be NULL");
+  CBM_CUDA(h, cudaSetDevice(h->cfg.device));
+  CBM_CUDA(h, cudaEventSynchronize(s.ev_d2h));  // the count came back with the results
+  const uint32_t n = *s.h_nsel;
+  *n_selected = n;
+  if (n > capacity) return fail(h, CBM_ERR_CAPACITY, "%u events selected, room for %u", n, capacity);
+  if (n) {
+    if (!event_ids) return fail(h, CBM_ERR_INVALID_ARG, "event_ids must not be NULL");
+    CBM_CUDA(h, cudaMemcpyAsync(event_ids, s.d_sel, (size_t)n * 4, cudaMemcpyDeviceToHost, h->st_d2h));
+    CBM_CUDA(h, cudaStreamSynchronize(h->st_d2h));
+  }
+  return CBM_OK;
+}
+
+int cbm_trigger_select_device(cbm_trigger_t* h, uint32_t n_events, const uint8_t* d_accept, uint32_t* d_event_ids,
+                              uint32_t* d_n_selected, void* stream) {
+  if (!h) return CBM_ERR_INVALID_ARG;
+  if (n_events > h->cfg.max_events) return fail(h, CBM_ERR_CAPACITY, "n_events %u > max_events %u", n_events, h->cfg.max_events);
+  if (!d_n_selected || (n_events && (!d_accept || !d_event_ids))) return fail(h, CBM_ERR_INVALID_ARG, "device pointers must not be NULL");
+  CBM_CUDA(h, cudaSetDevice(h->cfg.device));
+  const int nl = launch_compaction(h, h->dev_scr, d_accept, n_events, d_event_ids, d_n_selected, (cudaStream_t)stream);
+  return nl < 0 ? nl : CBM_OK;
 }
 
 int cbm_trigger_get_stats(cbm_trigger_t* h, uint32_t slot, cbm_trigger_stats_t* stats) {

@@ -290,7 +290,7 @@ def test_two_slot_pipeline_matches_per_batch():
         for i in (len(batches) - 2, len(batches) - 1):
             got[i] = trig.fetch_results(i & 1, 5000)
         st = trig.stats(0)
-        assert st.n_launches == 4 and st.kernel_ms[0] > 0 and st.h2d_ms > 0
+        assert st.n_launches == 6 and st.kernel_ms[0] > 0 and st.h2d_ms > 0  # 4 selection + 2 list kernels
     for i in range(len(batches)):
         assert_same(got[i], want[i], f"batch {i}")
 

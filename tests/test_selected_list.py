@@ -1,0 +1,110 @@
+"""The list of selected events.
+
+CPU: oracle.selected is pinned against numpy's flatnonzero and hand-written cases.
+GPU: cbm_trigger_fetch_selected / cbm_trigger_select_device against oracle.selected, bit-exact (index work).
+"""
+import numpy as np
+import pytest
+
+import oracle
+from paper_1810_11966_b200 import workloads as W
+
+
+# ------------------------------------------------------------------------------------------------ CPU pins
+def test_oracle_selected_hand_cases():
+    assert oracle.selected(np.zeros(0, dtype=np.uint8)).tolist() == []
+    assert oracle.selected(np.array([0, 0, 0], dtype=np.uint8)).tolist() == []
+    assert oracle.selected(np.array([1, 0, 1, 1, 0], dtype=np.uint8)).tolist() == [0, 2, 3]
+    assert oracle.selected(np.array([0, 0, 0, 0, 7], dtype=np.uint8)).tolist() == [4]  # any non-zero byte counts
+    assert oracle.selected(np.ones(5, dtype=np.uint8)).dtype == np.uint32
+
+
+def test_oracle_selected_against_library_routine():
+    rng = np.random.default_rng(11)
+    for n, p in ((1, 0.5), (17, 0.3), (4096, 0.01), (4097, 0.5), (10000, 0.999)):
+        a = (rng.random(n) < p).astype(np.uint8)
+        got = oracle.selected(a)
+        assert np.array_equal(got, np.flatnonzero(a).astype(np.uint32))
+        assert np.all(np.diff(got.astype(np.int64)) > 0)  # ascending, no duplicates
+        assert got.size == int(a.sum())
+
+
+def test_oracle_selected_is_the_accept_flags_of_the_oracle():
+    cfg = W.CONFIGS[0]
+    b = W.generate(cfg, n_events=400)
+    g = oracle.geometry(cfg.layer_z, cfg.win_in, cfg.win_link, cfg.min_candidates)
+    _, nc, ac = oracle.run(g, b.x, b.y, b.off)
+    ids = oracle.selected(ac)
+    assert ids.size > 0
+    assert np.all(nc[ids] >= cfg.min_candidates) and np.all(np.delete(nc, ids) < cfg.min_candidates)
+
+
+# ------------------------------------------------------------------------------------------------ GPU parity
+@pytest.mark.gpu
+@pytest.mark.parametrize("cid,n", [(0, 1000), (1, 3000), (3, 20000), (2, 1500)])
+def test_fetch_selected_matches_oracle(cid, n):
+    from paper_1810_11966_b200 import binding as K
+    from tests.helpers import oracle_mt
+    cfg = W.CONFIGS[cid]
+    b = W.generate(cfg, n_events=n)
+    g = oracle.geometry(cfg.layer_z, cfg.win_in, cfg.win_link, cfg.min_candidates)
+    _, _, oac = oracle_mt(g, b.x, b.y, b.off)
+    with K.Trigger(cfg.layer_z, n, b.n_hits, win_in=cfg.win_in, win_link=cfg.win_link,
+                   min_candidates=cfg.min_candidates, n_slots=1) as trig:
+        trig.upload_events(0, b.x, b.y, b.off)
+        trig.run(0)
+        ids_before = trig.fetch_selected(0)            # before fetch_results
+        _, _, ac = trig.fetch_results(0, n)
+        ids_after = trig.fetch_selected(0)             # and after it
+        assert np.array_equal(ac, oac)
+        want = oracle.selected(oac)
+        assert np.array_equal(ids_before, want) and np.array_equal(ids_after, want)
+        # too little room: the count is still reported, nothing is written
+        if want.size > 1:
+            with pytest.raises(K.CbmTriggerError) as ei:
+                trig.fetch_selected(0, capacity=want.size - 1)
+            assert ei.value.code == K.CBM_ERR_CAPACITY
+        # a new upload invalidates the list
+        trig.upload_events(0, b.x, b.y, b.off)
+        with pytest.raises(K.CbmTriggerError) as ei:
+            trig.fetch_selected(0)
+        assert ei.value.code == K.CBM_ERR_STATE
+
+
+@pytest.mark.gpu
+def test_fetch_selected_none_all_and_empty():
+    from paper_1810_11966_b200 import binding as K
+    cfg = W.CONFIGS[0]
+    b = W.generate(cfg, n_events=300)
+    # min_candidates = 0 accepts every event (B3); a huge threshold accepts none
+    for minc, want in ((0, np.arange(300, dtype=np.uint32)), (0xFFFFFFFF, np.zeros(0, dtype=np.uint32))):
+        with K.Trigger(cfg.layer_z, 300, b.n_hits, min_candidates=minc, n_slots=1) as trig:
+            trig.upload_events(0, b.x, b.y, b.off)
+            trig.run(0)
+            assert np.array_equal(trig.fetch_selected(0), want)
+    with K.Trigger(cfg.layer_z, 8, 8, n_slots=1) as trig:  # empty batch
+        trig.upload_events(0, np.zeros(0, np.int32), np.zeros(0, np.int32), np.zeros(1, np.uint32), 0, 0)
+        trig.run(0)
+        assert trig.fetch_selected(0).size == 0
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("n", [1, 15, 16, 4095, 4096, 4097, 70001])
+def test_select_device_on_arbitrary_flags(n):
+    """The compaction alone on device arrays: block boundaries (4096 events), ragged tails, unaligned start."""
+    import torch
+    from paper_1810_11966_b200 import binding as K
+    rng = np.random.default_rng(n)
+    cfg = W.CONFIGS[0]
+    with K.Trigger(cfg.layer_z, 80000, 16, n_slots=0) as trig:
+        for p, shift in ((0.02, 0), (0.5, 0), (1.0, 0), (0.3, 3)):
+            a = (rng.random(n + shift) < p).astype(np.uint8)
+            a[a != 0] = rng.integers(1, 256, size=int(a.sum()), dtype=np.uint8)  # any non-zero byte
+            d_a = torch.from_numpy(a).cuda()
+            d_ids = torch.full((n,), 0xFFFFFFF, dtype=torch.int32, device="cuda")
+            d_n = torch.zeros(1, dtype=torch.int32, device="cuda")
+            trig.select_device(n, d_a[shift:], d_ids, d_n)
+            torch.cuda.synchronize()
+            want = oracle.selected(a[shift:])
+            assert int(d_n.item()) == want.size
+            assert np.array_equal(d_ids.cpu().numpy().view(np.uint32)[:want.size], want)
