@@ -43,6 +43,7 @@ def parse_args():
     ap.add_argument("--e2e-steps", type=int, default=0, help="steps of the end-to-end leg (0 = min(steps, 10))")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-packed", action="store_true", help="skip the end-to-end leg with the packed wire format XY20")
     return ap.parse_args()
 
 
@@ -85,9 +86,11 @@ class ClockSampler:
         for line in self.proc.stdout:
             parts = [p.strip() for p in line.split(",")]
             if len(parts) >= 7:
-                self.samples.append(parts)
+                self.samples.append((time.perf_counter(), parts))
 
-    def stop(self):
+    def stop(self, t0=None, t1=None):
+        """Samples taken inside the timed region [t0, t1] (host clock); if the region was shorter than the
+        sampling interval, the samples of the surrounding loaded phase (warm-up included) are used."""
         if self.proc is None:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
         self.proc.terminate()
@@ -95,9 +98,14 @@ class ClockSampler:
             self.proc.wait(timeout=5)
         except Exception:
             self.proc.kill()
+        inside = [p for (t, p) in self.samples if t0 is not None and t0 <= t <= t1 + 0.03]
+        window = "timed region"
+        if len(inside) < 2:
+            inside, window = [p for (_, p) in self.samples], "warm-up + timed region"
         sm, mx, reasons = [], [], set()
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        for p in self.samples:
+        self.window = window
+        for p in inside:
             try:
                 sm.append(float(p[0]))
                 mx.append(float(p[1]))
@@ -107,7 +115,7 @@ class ClockSampler:
                 if v.lower().startswith("active"):
                     reasons.add(name)
         return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
-                "reasons": sorted(reasons), "samples": len(sm)}
+                "reasons": sorted(reasons), "samples": len(sm), "window": window}
 
 
 # ---------------------------------------------------------------------------------------------- accounting
@@ -267,21 +275,27 @@ def run_ours(args, cfg, cid):
                      device=local_rank, flags=K.CBM_FLAG_PROFILE)
     stream = torch.cuda.Stream(device=dev)
     sampler = ClockSampler(local_rank)
+    sampler.start()  # nvidia-smi needs ~0.1 s to deliver its first sample: started before the warm-up
     with torch.cuda.stream(stream):
-        for _ in range(args.warmup):
-            trig.run_device(E, n_hits, dx, dy, doff, dnt, dnc, dac)
+        t_load = time.perf_counter()
+        n_warm = 0
+        while n_warm < args.warmup or (time.perf_counter() - t_load < 0.25 and n_warm < 1000):
+            trig.run_device(E, n_hits, dx, dy, doff, dnt, dnc, dac)  # untimed: W steps, and at least 0.25 s of load
+            n_warm += 1
+            if n_warm >= args.warmup:
+                torch.cuda.synchronize()
         rc, st = trig.device_status()
         if rc != K.CBM_OK:
             raise SystemExit("bench.py: the device rejected events of a generated batch")
         barrier()
-        sampler.start()
         ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        t_region0 = time.perf_counter()
         ev0.record(stream)
         for _ in range(args.steps):
             trig.run_device(E, n_hits, dx, dy, doff, dnt, dnc, dac)
         ev1.record(stream)
         barrier()
-        clocks = sampler.stop()
+        clocks = sampler.stop(t_region0, time.perf_counter())
         ms_total = ev0.elapsed_time(ev1)
         ktimes = trig.device_kernel_times(n_last=args.steps)
     n_accept = int(dac.sum().item())
@@ -290,9 +304,11 @@ def run_ours(args, cfg, cid):
     trig.close()
 
     # ---- end-to-end leg: pinned HOST buffers -> H2D -> kernels -> D2H, two slots in flight
-    e2e = None
+    e2e = e2e_packed = None
     if not args.no_e2e:
         e2e = run_e2e(args, cfg, cid, batch, K, W, local_rank, rank, barrier)
+        if not args.no_packed and cfg.chunk_events == 0:
+            e2e_packed = run_e2e(args, cfg, cid, batch, K, W, local_rank, rank, barrier, packed=True)
     del dx, dy, doff
 
     # max over ranks (device time), whole-job aggregate
@@ -341,7 +357,7 @@ def run_ours(args, cfg, cid):
         "roofline": roofline,
         "roofline_step": {"bound": "hbm", "achieved": step_gbs, "peak": peak, "unit": "GB/s", "frac": step_gbs / peak,
                           "frac_of_8TBs_nominal": step_gbs / 8000.0, "algorithmic_bytes_per_step": B_alg},
-        "clocks": clocks, "generation_s": t_gen,
+        "clocks": clocks, "warmup_steps_run": n_warm, "generation_s": t_gen,
     }
     if e2e:
         e2e_value = whole_job_rate(events_all, e2e["steps"], e2e_s_max)
@@ -349,6 +365,13 @@ def run_ours(args, cfg, cid):
                       "d2h_bytes_per_step": e2e["d2h_bytes"], "steps": e2e["steps"], "slots": 2,
                       "ms_per_step": 1e3 * e2e_s_max / e2e["steps"], "h2d_gbs": e2e["h2d_bytes"] * e2e["steps"] / e2e_s_max / 1e9,
                       "vs_10MHz": e2e_value / CBM_INTERACTION_RATE_HZ, "h2d_ms_last": e2e["h2d_ms"], "kernel_ms_last": e2e["kernel_ms"]}
+    if e2e_packed and world == 1:  # extra: the same pipeline fed with the 5-byte-per-hit wire format
+        v = whole_job_rate(E, e2e_packed["steps"], e2e_packed["seconds"])
+        out["e2e_packed_xy20"] = {"value": v, "unit": UNIT, "h2d_bytes_per_step": e2e_packed["h2d_bytes"],
+                                  "d2h_bytes_per_step": e2e_packed["d2h_bytes"], "steps": e2e_packed["steps"],
+                                  "ms_per_step": 1e3 * e2e_packed["seconds"] / e2e_packed["steps"],
+                                  "h2d_gbs": e2e_packed["h2d_bytes"] * e2e_packed["steps"] / e2e_packed["seconds"] / 1e9,
+                                  "vs_10MHz": v / CBM_INTERACTION_RATE_HZ, "accepted": e2e_packed["accepted"]}
     if world == 1 and not args.no_cpu_baseline:
         n_threads = os.cpu_count() or 1
         n_sample = min(E, cpu_sample_size(cid))
@@ -366,7 +389,7 @@ NCU_TRAFFIC_BYTES = {
 }
 
 
-def run_e2e(args, cfg, cid, batch, K, W, local_rank, rank, barrier):
+def run_e2e(args, cfg, cid, batch, K, W, local_rank, rank, barrier, packed=False):
     """K2 batches through upload_events / run / fetch_results, inputs in the slots' pinned HOST buffers
     (cbm_trigger_host_buffers: the producer writes there), two slots in flight so that the H2D of batch i+1
     overlaps the kernels and the D2H of batch i.  Wall clock between device synchronisations."""
@@ -379,15 +402,21 @@ def run_e2e(args, cfg, cid, batch, K, W, local_rank, rank, barrier):
     max_hits = max(b.n_hits for b in batches)
     trig = K.Trigger(cfg.layer_z, E, max_hits, win_in=cfg.win_in, win_link=cfg.win_link,
                      min_candidates=cfg.min_candidates, max_hits_per_layer=cfg.max_hits_per_layer, n_slots=2,
-                     device=local_rank, flags=K.CBM_FLAG_PROFILE)
+                     device=local_rank, flags=K.CBM_FLAG_PROFILE | (K.CBM_FLAG_PACKED_INPUT if packed else 0))
     bufs, nh = [], []
-    for s in (0, 1):
+    for s in (0, 1):  # the producer (DAQ / generator) writes the batch into the slot's pinned staging, untimed
         b = batches[s % len(batches)]
-        hx, hy, ho = trig.host_buffers(s)
-        hx[:b.n_hits] = b.x
-        hy[:b.n_hits] = b.y
-        ho[:b.off.size] = b.off
-        bufs.append((hx, hy, ho))
+        if packed:
+            hp, ho = trig.host_buffers_packed(s)
+            hp[:5 * b.n_hits] = W.pack_xy20(b.x, b.y)
+            ho[:b.off.size] = b.off
+            bufs.append((hp, ho))
+        else:
+            hx, hy, ho = trig.host_buffers(s)
+            hx[:b.n_hits] = b.x
+            hy[:b.n_hits] = b.y
+            ho[:b.off.size] = b.off
+            bufs.append((hx, hy, ho))
         nh.append(b.n_hits)
     out = [(np.empty((E, S), dtype=np.uint32), np.empty(E, dtype=np.uint32), np.empty(E, dtype=np.uint8)) for _ in (0, 1)]
 
@@ -396,7 +425,10 @@ def run_e2e(args, cfg, cid, batch, K, W, local_rank, rank, barrier):
             s = i & 1
             if i >= 2:
                 trig.fetch_results(s, E, out=out[s])
-            trig.upload_events(s, bufs[s][0], bufs[s][1], bufs[s][2], E, nh[s])
+            if packed:
+                trig.upload_events_packed(s, bufs[s][0], bufs[s][1], E, nh[s])
+            else:
+                trig.upload_events(s, bufs[s][0], bufs[s][1], bufs[s][2], E, nh[s])
             trig.run(s)
         for i in range(max(0, n - 2), n):
             trig.fetch_results(i & 1, E, out=out[i & 1])
@@ -408,7 +440,8 @@ def run_e2e(args, cfg, cid, batch, K, W, local_rank, rank, barrier):
     torch.cuda.synchronize()
     dt = time.perf_counter() - t0
     st = trig.stats(0)
-    res = {"seconds": dt, "steps": steps, "h2d_bytes": 8 * nh[0] + 4 * (E * L + 1), "d2h_bytes": E * (4 * S + 5) + 64,
+    hit_bytes = 20 * ((nh[0] + 3) // 4) if packed else 8 * nh[0]
+    res = {"seconds": dt, "steps": steps, "h2d_bytes": hit_bytes + 4 * (E * L + 1), "d2h_bytes": E * (4 * S + 5) + 64 + 4,
            "h2d_ms": float(st.h2d_ms), "kernel_ms": [float(v) for v in st.kernel_ms], "accepted": int(out[0][2].sum())}
     trig.close()
     return res

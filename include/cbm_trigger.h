@@ -81,6 +81,7 @@ typedef struct {
 
 #define CBM_FLAG_PROFILE 1u      /* record CUDA events around every kernel (cbm_trigger_get_stats: kernel_ms) */
 #define CBM_FLAG_NO_TINY_PATH 2u /* tuning/testing: route every event through the team kernels */
+#define CBM_FLAG_PACKED_INPUT 4u /* the slots take the packed wire format XY20 (cbm_trigger_upload_events_packed) */
 
 typedef struct {
   uint32_t struct_size;
@@ -116,6 +117,18 @@ int cbm_trigger_host_buffers(cbm_trigger_t* h, uint32_t slot, int32_t** x, int32
  * PAPER.md:160-161 "allocate memory on the device ... transfer the data from host to device". */
 int cbm_trigger_upload_events(cbm_trigger_t* h, uint32_t slot, uint32_t n_events, uint64_t n_hits,
                               const int32_t* x, const int32_t* y, const uint32_t* off);
+
+/* Packed wire format XY20 (shrinking the transfer was the paper's biggest
+ * win): 5 bytes per hit instead of 8.  xy20[5*i .. 5*i+4] holds hit i of x[] / y[], little endian: bits 0..19 = x,
+ * bits 20..39 = y, each 20-bit two's complement (10-um units, -524288 <= v <= 524287; a producer with larger
+ * coordinates must use the int32 format).  A handle created with CBM_FLAG_PACKED_INPUT stages and copies the
+ * packed stream (n_hits*5 bytes, rounded up to 20) and `run` first expands it on the device into the int32
+ * arrays the kernels read; results are identical to uploading the same hits as int32.  Such a handle accepts
+ * only the packed calls (the int32 ones return CBM_ERR_STATE) and vice versa.  Otherwise as
+ * cbm_trigger_host_buffers / cbm_trigger_upload_events.  xy20: HOST (capacity max_hits*5 bytes), off: HOST. */
+int cbm_trigger_host_buffers_packed(cbm_trigger_t* h, uint32_t slot, uint8_t** xy20, uint32_t** off);
+int cbm_trigger_upload_events_packed(cbm_trigger_t* h, uint32_t slot, uint32_t n_events, uint64_t n_hits,
+                                     const uint8_t* xy20, const uint32_t* off);
 
 /* a3-a8: enqueue the selection kernels for the batch in `slot` after its H2D, and the D2H of the results after
  * the kernels (separate streams, event-ordered).  Returns immediately.

@@ -140,3 +140,18 @@ def selected(accept):
         if a:
             ids.append(e)
     return np.asarray(ids, dtype=np.uint32)
+
+
+def unpack_xy20(xy20):
+    """The packed wire format XY20 (include/cbm_trigger.h), decoded hit by hit:
+    bytes 5i..5i+4 of the stream, little endian, hold x in bits 0..19 and y in bits 20..39, each a 20-bit
+    two's complement number.  Returns (x, y) as int32 arrays."""
+    b = list(bytes(xy20)) if isinstance(xy20, (bytes, bytearray)) else np.asarray(xy20, dtype=np.uint8).ravel().tolist()
+    n = len(b) // 5
+    xs, ys = [], []
+    for i in range(n):
+        v = b[5 * i] | (b[5 * i + 1] << 8) | (b[5 * i + 2] << 16) | (b[5 * i + 3] << 24) | (b[5 * i + 4] << 32)
+        xv, yv = v & 0xFFFFF, (v >> 20) & 0xFFFFF
+        xs.append(xv - (1 << 20) if xv >= (1 << 19) else xv)
+        ys.append(yv - (1 << 20) if yv >= (1 << 19) else yv)
+    return np.asarray(xs, dtype=np.int32), np.asarray(ys, dtype=np.int32)

@@ -18,12 +18,13 @@ MAX_LAYERS = 24
 N_KERNELS = 4
 KERNEL_NAMES = ("tile_kernel", "team_kernel_M", "team_kernel_H", "team_kernel_G")
 CBM_OK, CBM_ERR_INVALID_ARG, CBM_ERR_RANGE, CBM_ERR_CAPACITY, CBM_ERR_STATE, CBM_ERR_CUDA = 0, -1, -2, -3, -4, -5
-CBM_FLAG_PROFILE, CBM_FLAG_NO_TINY_PATH = 1, 2
+CBM_FLAG_PROFILE, CBM_FLAG_NO_TINY_PATH, CBM_FLAG_PACKED_INPUT = 1, 2, 4
 EXPORTS = (
     "cbm_trigger_create", "cbm_trigger_destroy", "cbm_trigger_host_buffers", "cbm_trigger_upload_events",
     "cbm_trigger_run", "cbm_trigger_fetch_results", "cbm_trigger_run_device", "cbm_trigger_device_status",
     "cbm_trigger_get_stats", "cbm_trigger_last_error", "cbm_trigger_version", "cbm_trigger_device_kernel_times",
     "cbm_trigger_fetch_selected", "cbm_trigger_select_device",
+    "cbm_trigger_host_buffers_packed", "cbm_trigger_upload_events_packed",
 )
 PROFILE_RING = 32
 # scheduler classes (csrc/cbm_trigger.cu, csrc/params.h), restated for bookkeeping in bench.py only
@@ -96,6 +97,10 @@ def load_library():
         lib.cbm_trigger_host_buffers.argtypes = [vp, u32, ctypes.POINTER(vp), ctypes.POINTER(vp), ctypes.POINTER(vp)]
         lib.cbm_trigger_upload_events.restype = i32
         lib.cbm_trigger_upload_events.argtypes = [vp, u32, u32, u64, vp, vp, vp]
+        lib.cbm_trigger_host_buffers_packed.restype = i32
+        lib.cbm_trigger_host_buffers_packed.argtypes = [vp, u32, ctypes.POINTER(vp), ctypes.POINTER(vp)]
+        lib.cbm_trigger_upload_events_packed.restype = i32
+        lib.cbm_trigger_upload_events_packed.argtypes = [vp, u32, u32, u64, vp, vp]
         lib.cbm_trigger_run.restype = i32
         lib.cbm_trigger_run.argtypes = [vp, u32]
         lib.cbm_trigger_fetch_results.restype = i32
@@ -182,6 +187,20 @@ def _host_ptr(a, dtype):
 def cbm_trigger_upload_events(handle, slot, n_events, n_hits, x, y, off):
     _check(load_library().cbm_trigger_upload_events(handle, slot, n_events, n_hits, _host_ptr(x, np.int32),
                                                     _host_ptr(y, np.int32), _host_ptr(off, np.uint32)), handle)
+
+
+def cbm_trigger_host_buffers_packed(handle, slot, max_hits, n_off):
+    """numpy views (no copy) of the slot's pinned staging buffers of the packed wire format XY20."""
+    pp, po = ctypes.c_void_p(), ctypes.c_void_p()
+    _check(load_library().cbm_trigger_host_buffers_packed(handle, slot, ctypes.byref(pp), ctypes.byref(po)), handle)
+    xy = np.ctypeslib.as_array(ctypes.cast(pp, ctypes.POINTER(ctypes.c_uint8)), shape=(max(int(max_hits), 1) * 5,))
+    off = np.ctypeslib.as_array(ctypes.cast(po, ctypes.POINTER(ctypes.c_uint32)), shape=(int(n_off),))
+    return xy, off
+
+
+def cbm_trigger_upload_events_packed(handle, slot, n_events, n_hits, xy20, off):
+    _check(load_library().cbm_trigger_upload_events_packed(handle, slot, n_events, n_hits, _host_ptr(xy20, np.uint8),
+                                                           _host_ptr(off, np.uint32)), handle)
 
 
 def cbm_trigger_run(handle, slot):
@@ -276,6 +295,15 @@ class Trigger:
         n_events = (off.size - 1) // self.L if n_events is None else n_events
         n_hits = int(off[n_events * self.L]) if n_hits is None else n_hits
         cbm_trigger_upload_events(self.handle, slot, n_events, n_hits, x, y, off)
+        return n_events, n_hits
+
+    def host_buffers_packed(self, slot):
+        return cbm_trigger_host_buffers_packed(self.handle, slot, self.cfg.max_hits, self.cfg.max_events * self.L + 1)
+
+    def upload_events_packed(self, slot, xy20, off, n_events=None, n_hits=None):
+        n_events = (off.size - 1) // self.L if n_events is None else n_events
+        n_hits = int(off[n_events * self.L]) if n_hits is None else n_hits
+        cbm_trigger_upload_events_packed(self.handle, slot, n_events, n_hits, xy20, off)
         return n_events, n_hits
 
     def run(self, slot):

@@ -17,6 +17,7 @@
 #include "../../include/cbm_trigger.h"
 #include "kernels.cuh"
 #include "select.cuh"
+#include "wire.cuh"
 
 namespace {
 
@@ -52,6 +53,9 @@ struct ProfEvents {
 
 struct Slot {
   int32_t *h_x = nullptr, *h_y = nullptr;
+  uint8_t* h_p = nullptr;   // CBM_FLAG_PACKED_INPUT: pinned staging of the XY20 stream (instead of h_x, h_y)
+  uint32_t* d_p = nullptr;  // ... and its device copy, expanded into d_x, d_y by `run`
+  bool packed_pending = false;
   uint32_t* h_off = nullptr;
   int32_t *d_x = nullptr, *d_y = nullptr;
   uint32_t* d_off = nullptr;
@@ -228,8 +232,13 @@ int alloc_slot(cbm_trigger* h, Slot& s) {
   const size_t nh = (size_t)((c.max_hits + 3) & ~3ull) + 4;  // 16-byte tail padding for the bulk copies
   const size_t noff = (size_t)c.max_events * h->p.L + 1;
   const size_t ne = c.max_events, S = h->p.S;
-  CBM_CUDA(h, cudaHostAlloc(&s.h_x, nh * 4, cudaHostAllocDefault));
-  CBM_CUDA(h, cudaHostAlloc(&s.h_y, nh * 4, cudaHostAllocDefault));
+  if (c.flags & CBM_FLAG_PACKED_INPUT) {
+    CBM_CUDA(h, cudaHostAlloc(&s.h_p, nh * 5, cudaHostAllocDefault));  // nh is a multiple of 4: whole 20-byte groups
+    CBM_CUDA(h, cudaMalloc(&s.d_p, nh * 5));
+  } else {
+    CBM_CUDA(h, cudaHostAlloc(&s.h_x, nh * 4, cudaHostAllocDefault));
+    CBM_CUDA(h, cudaHostAlloc(&s.h_y, nh * 4, cudaHostAllocDefault));
+  }
   CBM_CUDA(h, cudaHostAlloc(&s.h_off, noff * 4, cudaHostAllocDefault));
   CBM_CUDA(h, cudaMalloc(&s.d_x, nh * 4));
   CBM_CUDA(h, cudaMalloc(&s.d_y, nh * 4));
@@ -256,6 +265,7 @@ int alloc_slot(cbm_trigger* h, Slot& s) {
 }
 void free_slot(Slot& s) {
   cudaFreeHost(s.h_x); cudaFreeHost(s.h_y); cudaFreeHost(s.h_off);
+  cudaFreeHost(s.h_p); cudaFree(s.d_p);
   cudaFree(s.d_x); cudaFree(s.d_y); cudaFree(s.d_off);
   cudaFree(s.d_nt); cudaFree(s.d_nc); cudaFree(s.d_ac);
   cudaFree(s.d_sel); cudaFree(s.d_nsel); cudaFreeHost(s.h_nsel);
@@ -457,6 +467,7 @@ int cbm_trigger_host_buffers(cbm_trigger_t* h, uint32_t slot, int32_t** x, int32
   int rc = check_slot(h, slot);
   if (rc) return rc;
   if (!x || !y || !off) return fail(h, CBM_ERR_INVALID_ARG, "x, y, off must not be NULL");
+  if (h->cfg.flags & CBM_FLAG_PACKED_INPUT) return fail(h, CBM_ERR_STATE, "the handle takes packed input (CBM_FLAG_PACKED_INPUT)");
   *x = h->slot[slot].h_x; *y = h->slot[slot].h_y; *off = h->slot[slot].h_off;
   return CBM_OK;
 }
@@ -466,6 +477,7 @@ int cbm_trigger_upload_events(cbm_trigger_t* h, uint32_t slot, uint32_t n_events
   int rc = check_slot(h, slot);
   if (rc) return rc;
   Slot& s = h->slot[slot];
+  if (h->cfg.flags & CBM_FLAG_PACKED_INPUT) return fail(h, CBM_ERR_STATE, "the handle takes packed input (CBM_FLAG_PACKED_INPUT)");
   if (!off || (n_hits && (!x || !y))) return fail(h, CBM_ERR_INVALID_ARG, "x, y, off must not be NULL");
   if (n_events > h->cfg.max_events) return fail(h, CBM_ERR_CAPACITY, "n_events %u > max_events %u", n_events, h->cfg.max_events);
   if (n_hits > h->cfg.max_hits) return fail(h, CBM_ERR_CAPACITY, "n_hits %llu > max_hits %llu", (unsigned long long)n_hits, (unsigned long long)h->cfg.max_hits);
@@ -497,6 +509,48 @@ int cbm_trigger_upload_events(cbm_trigger_t* h, uint32_t slot, uint32_t n_events
   return CBM_OK;
 }
 
+int cbm_trigger_host_buffers_packed(cbm_trigger_t* h, uint32_t slot, uint8_t** xy20, uint32_t** off) {
+  int rc = check_slot(h, slot);
+  if (rc) return rc;
+  if (!xy20 || !off) return fail(h, CBM_ERR_INVALID_ARG, "xy20, off must not be NULL");
+  if (!(h->cfg.flags & CBM_FLAG_PACKED_INPUT)) return fail(h, CBM_ERR_STATE, "the handle was created without CBM_FLAG_PACKED_INPUT");
+  *xy20 = h->slot[slot].h_p; *off = h->slot[slot].h_off;
+  return CBM_OK;
+}
+
+int cbm_trigger_upload_events_packed(cbm_trigger_t* h, uint32_t slot, uint32_t n_events, uint64_t n_hits,
+                                     const uint8_t* xy20, const uint32_t* off) {
+  int rc = check_slot(h, slot);
+  if (rc) return rc;
+  Slot& s = h->slot[slot];
+  if (!(h->cfg.flags & CBM_FLAG_PACKED_INPUT)) return fail(h, CBM_ERR_STATE, "the handle was created without CBM_FLAG_PACKED_INPUT");
+  if (!off || (n_hits && !xy20)) return fail(h, CBM_ERR_INVALID_ARG, "xy20, off must not be NULL");
+  if (n_events > h->cfg.max_events) return fail(h, CBM_ERR_CAPACITY, "n_events %u > max_events %u", n_events, h->cfg.max_events);
+  if (n_hits > h->cfg.max_hits) return fail(h, CBM_ERR_CAPACITY, "n_hits %llu > max_hits %llu", (unsigned long long)n_hits, (unsigned long long)h->cfg.max_hits);
+  if (s.state == kRunning) return fail(h, CBM_ERR_STATE, "slot %u holds unfetched results", slot);
+  const size_t n_off = (size_t)n_events * h->p.L + 1;
+  if (off[0] != 0 || off[n_off - 1] != n_hits)
+    return fail(h, CBM_ERR_RANGE, "off[0] must be 0 and off[n_events*L] must equal n_hits");
+  CBM_CUDA(h, cudaSetDevice(h->cfg.device));
+  CBM_CUDA(h, cudaEventSynchronize(s.ev_h2d));  // the staging buffers may still be the source of the previous H2D
+  const size_t n_bytes = (size_t)n_hits * 5, n_copy = (size_t)((n_hits + 3) / 4) * 20;  // whole 20-byte groups
+  if (xy20 != s.h_p && n_hits) memcpy(s.h_p, xy20, n_bytes);
+  if (off != s.h_off) memcpy(s.h_off, off, n_off * 4);
+  CBM_CUDA(h, cudaStreamWaitEvent(h->st_h2d, s.ev_run, 0));  // the device arrays may still be read by the previous kernels
+  const bool prof = h->cfg.flags & CBM_FLAG_PROFILE;
+  if (prof) CBM_CUDA(h, cudaEventRecord(s.prof.h2d[0], h->st_h2d));
+  if (n_hits) CBM_CUDA(h, cudaMemcpyAsync(s.d_p, s.h_p, n_copy, cudaMemcpyHostToDevice, h->st_h2d));
+  CBM_CUDA(h, cudaMemcpyAsync(s.d_off, s.h_off, n_off * 4, cudaMemcpyHostToDevice, h->st_h2d));
+  if (prof) CBM_CUDA(h, cudaEventRecord(s.prof.h2d[1], h->st_h2d));
+  CBM_CUDA(h, cudaEventRecord(s.ev_h2d, h->st_h2d));
+  s.n_events = n_events;
+  s.n_hits = n_hits;
+  s.sel_valid = false;
+  s.packed_pending = true;
+  s.state = kUploaded;
+  return CBM_OK;
+}
+
 int cbm_trigger_run(cbm_trigger_t* h, uint32_t slot) {
   int rc = check_slot(h, slot);
   if (rc) return rc;
@@ -506,6 +560,15 @@ int cbm_trigger_run(cbm_trigger_t* h, uint32_t slot) {
   const bool prof = h->cfg.flags & CBM_FLAG_PROFILE;
   CBM_CUDA(h, cudaStreamWaitEvent(h->st_run, s.ev_h2d, 0));
   CBM_CUDA(h, cudaStreamWaitEvent(h->st_run, s.ev_d2h, 0));  // previous results of this slot must have left
+  if (s.packed_pending) {  // a2': expand the XY20 stream into the int32 arrays the kernels read
+    if (s.n_hits) {
+      const uint64_t groups = (s.n_hits + 3) / 4;
+      unpack_xy20_kernel<<<(unsigned)((groups + kWireThreads - 1) / kWireThreads), kWireThreads, 0, h->st_run>>>(
+          s.d_p, s.n_hits, s.d_x, s.d_y);
+      CBM_CUDA(h, cudaGetLastError());
+    }
+    s.packed_pending = false;
+  }
   const int nl = launch_selection(h, s.scr, s.d_x, s.d_y, s.d_off, s.n_events, s.n_hits, s.d_nt, s.d_nc, s.d_ac,
                                   h->st_run, prof ? &s.prof : nullptr);
   if (nl < 0) return nl;

@@ -224,3 +224,17 @@ def batch_from_layers(layer_z, events) -> tuple:
             off.append(len(xs))
     return (np.asarray(xs, dtype=np.int32).reshape(-1), np.asarray(ys, dtype=np.int32).reshape(-1),
             np.asarray(off, dtype=np.uint32))
+
+
+XY20_MIN, XY20_MAX = -(1 << 19), (1 << 19) - 1
+
+
+def pack_xy20(x, y):
+    """The packed wire format XY20 of include/cbm_trigger.h (input formatting only): 5 bytes per hit, little
+    endian, bits 0..19 = x, bits 20..39 = y, 20-bit two's complement.  Raises if a coordinate does not fit."""
+    x = np.ascontiguousarray(x, dtype=np.int32)
+    y = np.ascontiguousarray(y, dtype=np.int32)
+    if x.size and (min(x.min(), y.min()) < XY20_MIN or max(x.max(), y.max()) > XY20_MAX):
+        raise ValueError("coordinate outside the 20-bit range of the XY20 wire format")
+    v = (x.astype(np.int64) & 0xFFFFF).astype(np.uint64) | ((y.astype(np.int64) & 0xFFFFF).astype(np.uint64) << np.uint64(20))
+    return np.ascontiguousarray(v.astype("<u8").view(np.uint8).reshape(-1, 8)[:, :5]).reshape(-1)
