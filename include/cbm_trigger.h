@@ -157,6 +157,28 @@ int cbm_trigger_fetch_selected(cbm_trigger_t* h, uint32_t slot, uint32_t* event_
 int cbm_trigger_select_device(cbm_trigger_t* h, uint32_t n_events, const uint8_t* d_accept, uint32_t* d_event_ids,
                               uint32_t* d_n_selected, void* stream);
 
+/* The paper's own selection, literally (section 3.2), on caller-owned DEVICE
+ * arrays (layout and stream as cbm_trigger_run_device; geometry = the handle's layer_z):
+ *   1. all triplets of the trigger station, one hit from each layer
+ *   2. least-squares line through the event vertex (0,0) in x-z and in y-z (x = m0 z, y = m1 z), mean square
+ *      deviation per degree of freedom <= thr_x (0.03) in x-z and <= thr_y (0.025) in y-z
+ *   3. d_accept[e] = d_n_passing[e] >= min_triplets (2)
+ * evaluated exactly: with Svz = sum v_i z_i, Szz = sum z_i^2, Svv = sum v_i^2 over the three hits,
+ *   den * (Szz*Svv - Svz^2) <= num * 10^6 * ndf * Szz      (thr = num/den cm^2; 10-um units; 128-bit integers),
+ * which needs |x|, |y| <= 2^23.  d_n_passing[n_events] uint32 = min(2^32-1, passing triplets); d_accept uint8.
+ * An event with malformed offsets selects nothing.  Asynchronous. */
+typedef struct {
+  uint32_t struct_size;            /* = sizeof(cbm_trigger_msd_params_t) */
+  uint32_t station;                /* the trigger station, 0..S-1; 0xFFFFFFFF = the last one */
+  uint32_t thr_x_num, thr_x_den;   /* MSD_xz threshold in cm^2 (0.03 = 3/100); den 1..4096, num <= 2^20 */
+  uint32_t thr_y_num, thr_y_den;   /* MSD_yz threshold (0.025 = 25/1000) */
+  uint32_t ndf;                    /* degrees of freedom, 1..16 (2: three hits, one fitted slope) */
+  uint32_t min_triplets;           /* 2 */
+} cbm_trigger_msd_params_t;
+int cbm_trigger_msd_device(cbm_trigger_t* h, const cbm_trigger_msd_params_t* params, uint32_t n_events, uint64_t n_hits,
+                           const int32_t* d_x, const int32_t* d_y, const uint32_t* d_off, uint32_t* d_n_passing,
+                           uint8_t* d_accept, void* stream);
+
 /* Device-resident entry point (PyTorch or any other owner of device memory and streams supplies both):
  * runs a3-a8 on caller-owned DEVICE arrays on the caller's stream (`stream` is a cudaStream_t passed as void*;
  * NULL = the legacy default stream).  d_x, d_y: n_hits int32 each, 16-byte aligned, readable up to the next

@@ -18,7 +18,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB = os.path.join(_HERE, "liboracle.so")
-_SRCS = [os.path.join(_HERE, "cbm_oracle.c"), os.path.join(_HERE, "slope_sorted.c")]
+_SRCS = [os.path.join(_HERE, "cbm_oracle.c"), os.path.join(_HERE, "slope_sorted.c"), os.path.join(_HERE, "msd_oracle.c")]
 MAX_LAYERS = 24
 
 
@@ -44,6 +44,33 @@ def geometry(layer_z, win_in=(1, 100), win_link=(2, 100), min_candidates=2) -> G
     return g
 
 
+class MsdParams(ctypes.Structure):
+    """Parameters of the paper-literal selection (oracle/msd_oracle.c)."""
+    _fields_ = [
+        ("n_stations", ctypes.c_uint32),
+        ("layer_z", ctypes.c_int32 * MAX_LAYERS),
+        ("station", ctypes.c_uint32),
+        ("thr_x_num", ctypes.c_uint32), ("thr_x_den", ctypes.c_uint32),
+        ("thr_y_num", ctypes.c_uint32), ("thr_y_den", ctypes.c_uint32),
+        ("ndf", ctypes.c_uint32),
+        ("min_triplets", ctypes.c_uint32),
+    ]
+
+
+def msd_params(layer_z, station=None, thr_x=(3, 100), thr_y=(25, 1000), ndf=2, min_triplets=2) -> MsdParams:
+    """MSD thresholds 0.03 (x-z) and 0.025 (y-z); at least two passing triplets."""
+    p = MsdParams()
+    assert len(layer_z) % 3 == 0 and 3 <= len(layer_z) <= MAX_LAYERS
+    p.n_stations = len(layer_z) // 3
+    for i, z in enumerate(layer_z):
+        p.layer_z[i] = int(z)
+    p.station = p.n_stations - 1 if station is None else station
+    p.thr_x_num, p.thr_x_den = thr_x
+    p.thr_y_num, p.thr_y_den = thr_y
+    p.ndf, p.min_triplets = ndf, min_triplets
+    return p
+
+
 def build(force: bool = False) -> str:
     """gcc -O2 (the paper's CPU flags, minus -march=native so the .so is portable)."""
     newest = max(os.path.getmtime(s) for s in _SRCS)
@@ -65,6 +92,8 @@ def _load():
         lib.cbm_oracle_run.argtypes = [ctypes.POINTER(Geometry), vp, vp, vp, u64, u64, u64, vp, vp, vp]
         lib.cbm_oracle_run_list.restype = ctypes.c_int
         lib.cbm_oracle_run_list.argtypes = [ctypes.POINTER(Geometry), vp, vp, vp, vp, u64, u64, vp, vp, vp]
+        lib.cbm_msd_oracle_run.restype = ctypes.c_int
+        lib.cbm_msd_oracle_run.argtypes = [ctypes.POINTER(MsdParams), vp, vp, vp, u64, u64, vp, vp]
         lib.cbm_slope_sorted_run.restype = ctypes.c_int
         lib.cbm_slope_sorted_run.argtypes = [ctypes.POINTER(Geometry), vp, vp, vp, u64, u64, vp, vp, vp, vp]
         _lib = lib
@@ -155,3 +184,20 @@ def unpack_xy20(xy20):
         xs.append(xv - (1 << 20) if xv >= (1 << 19) else xv)
         ys.append(yv - (1 << 20) if yv >= (1 << 19) else yv)
     return np.asarray(xs, dtype=np.int32), np.asarray(ys, dtype=np.int32)
+
+
+def run_msd(par: MsdParams, x, y, off, e_begin=0, e_end=None):
+    """The paper's selection, literally: triplets of the trigger station, least-squares line
+    through the vertex, MSD cut, at least two passing triplets.  Returns (n_passing[n], accept[n])."""
+    lib = _load()
+    x, y, off = _check_inputs(x, y, off)
+    n_events = (off.size - 1) // (3 * par.n_stations)
+    e_end = n_events if e_end is None else e_end
+    n = max(e_end - e_begin, 0)
+    npass = np.zeros(n, dtype=np.uint32)
+    ac = np.zeros(n, dtype=np.uint8)
+    rc = lib.cbm_msd_oracle_run(ctypes.byref(par), x.ctypes.data, y.ctypes.data, off.ctypes.data, e_begin, e_end,
+                                npass.ctypes.data, ac.ctypes.data)
+    if rc != 0:
+        raise RuntimeError(f"cbm_msd_oracle_run failed: {rc}")
+    return npass, ac

@@ -36,8 +36,7 @@
  * (|T_s| = n0*n1*n2, candidates = prod |T_s|, saturation); permutation invariance;
  * zero on constructed non-collinear noise; the independent slope-sorted counter
  * (oracle/slope_sorted.c); the closed-form uniform-background triplet rate.
- * The MSD thresholds of PAPER.md:76 are not part of this oracle: parity unpinned
- * for them (they need the paper's datasets).
+ * The paper's literal MSD cut is a separate oracle: oracle/msd_oracle.c.
  */
 #include <stdint.h>
 #include <stdlib.h>

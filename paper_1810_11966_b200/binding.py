@@ -24,7 +24,7 @@ EXPORTS = (
     "cbm_trigger_run", "cbm_trigger_fetch_results", "cbm_trigger_run_device", "cbm_trigger_device_status",
     "cbm_trigger_get_stats", "cbm_trigger_last_error", "cbm_trigger_version", "cbm_trigger_device_kernel_times",
     "cbm_trigger_fetch_selected", "cbm_trigger_select_device",
-    "cbm_trigger_host_buffers_packed", "cbm_trigger_upload_events_packed",
+    "cbm_trigger_host_buffers_packed", "cbm_trigger_upload_events_packed", "cbm_trigger_msd_device",
 )
 PROFILE_RING = 32
 # scheduler classes (csrc/cbm_trigger.cu, csrc/params.h), restated for bookkeeping in bench.py only
@@ -71,6 +71,27 @@ class Stats(ctypes.Structure):
                 "d2h_ms": float(self.d2h_ms)}
 
 
+class MsdParams(ctypes.Structure):
+    _fields_ = [
+        ("struct_size", ctypes.c_uint32),
+        ("station", ctypes.c_uint32),
+        ("thr_x_num", ctypes.c_uint32), ("thr_x_den", ctypes.c_uint32),
+        ("thr_y_num", ctypes.c_uint32), ("thr_y_den", ctypes.c_uint32),
+        ("ndf", ctypes.c_uint32),
+        ("min_triplets", ctypes.c_uint32),
+    ]
+
+
+def make_msd_params(station=None, thr_x=(3, 100), thr_y=(25, 1000), ndf=2, min_triplets=2) -> MsdParams:
+    m = MsdParams()
+    m.struct_size = ctypes.sizeof(MsdParams)
+    m.station = 0xFFFFFFFF if station is None else station
+    m.thr_x_num, m.thr_x_den = thr_x
+    m.thr_y_num, m.thr_y_den = thr_y
+    m.ndf, m.min_triplets = ndf, min_triplets
+    return m
+
+
 class CbmTriggerError(RuntimeError):
     def __init__(self, code, msg):
         super().__init__(f"cbm_trigger error {code}: {msg}")
@@ -115,6 +136,8 @@ def load_library():
         lib.cbm_trigger_fetch_selected.argtypes = [vp, u32, vp, u32, ctypes.POINTER(u32)]
         lib.cbm_trigger_select_device.restype = i32
         lib.cbm_trigger_select_device.argtypes = [vp, u32, vp, vp, vp, vp]
+        lib.cbm_trigger_msd_device.restype = i32
+        lib.cbm_trigger_msd_device.argtypes = [vp, ctypes.POINTER(MsdParams), u32, u64, vp, vp, vp, vp, vp, vp]
         lib.cbm_trigger_get_stats.restype = i32
         lib.cbm_trigger_get_stats.argtypes = [vp, u32, ctypes.POINTER(Stats)]
         lib.cbm_trigger_last_error.restype = ctypes.c_char_p
@@ -231,6 +254,12 @@ def cbm_trigger_select_device(handle, n_events, d_accept, d_event_ids, d_n_selec
     _check(load_library().cbm_trigger_select_device(handle, n_events, d_accept, d_event_ids, d_n_selected, stream), handle)
 
 
+def cbm_trigger_msd_device(handle, params, n_events, n_hits, d_x, d_y, d_off, d_n_passing, d_accept, stream=0):
+    """d_* are raw device addresses (ints); stream is a cudaStream_t as int."""
+    _check(load_library().cbm_trigger_msd_device(handle, ctypes.byref(params), n_events, n_hits, d_x, d_y, d_off,
+                                                 d_n_passing, d_accept, stream), handle)
+
+
 def cbm_trigger_get_stats(handle, slot) -> Stats:
     st = Stats()
     _check(load_library().cbm_trigger_get_stats(handle, slot, ctypes.byref(st)), handle)
@@ -344,6 +373,13 @@ class Trigger:
         st = torch.cuda.current_stream().cuda_stream if stream is None else stream
         cbm_trigger_run_device(self.handle, n_events, n_hits, d_x.data_ptr(), d_y.data_ptr(), d_off.data_ptr(),
                                d_nt.data_ptr(), d_nc.data_ptr(), d_ac.data_ptr(), st)
+
+    def msd_device(self, params, n_events, n_hits, d_x, d_y, d_off, d_np, d_ac, stream=None):
+        """The paper-literal selection on torch CUDA tensors."""
+        import torch
+        st = torch.cuda.current_stream().cuda_stream if stream is None else stream
+        cbm_trigger_msd_device(self.handle, params, n_events, n_hits, d_x.data_ptr(), d_y.data_ptr(), d_off.data_ptr(),
+                               d_np.data_ptr(), d_ac.data_ptr(), st)
 
     def device_kernel_times(self, stream=None, n_last=PROFILE_RING):
         import torch

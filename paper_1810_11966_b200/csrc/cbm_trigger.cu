@@ -18,6 +18,7 @@
 #include "kernels.cuh"
 #include "select.cuh"
 #include "wire.cuh"
+#include "msd.cuh"
 
 namespace {
 
@@ -646,6 +647,39 @@ int cbm_trigger_select_device(cbm_trigger_t* h, uint32_t n_events, const uint8_t
   CBM_CUDA(h, cudaSetDevice(h->cfg.device));
   const int nl = launch_compaction(h, h->dev_scr, d_accept, n_events, d_event_ids, d_n_selected, (cudaStream_t)stream);
   return nl < 0 ? nl : CBM_OK;
+}
+
+int cbm_trigger_msd_device(cbm_trigger_t* h, const cbm_trigger_msd_params_t* mp, uint32_t n_events, uint64_t n_hits,
+                           const int32_t* d_x, const int32_t* d_y, const uint32_t* d_off, uint32_t* d_n_passing,
+                           uint8_t* d_accept, void* stream) {
+  if (!h) return CBM_ERR_INVALID_ARG;
+  if (!mp || mp->struct_size != sizeof(cbm_trigger_msd_params_t)) return fail(h, CBM_ERR_INVALID_ARG, "msd params: NULL or bad struct_size");
+  const uint32_t st = mp->station == 0xFFFFFFFFu ? h->p.S - 1 : mp->station;
+  if (st >= h->p.S) return fail(h, CBM_ERR_INVALID_ARG, "msd params: station %u of %u", mp->station, h->p.S);
+  if (mp->thr_x_den == 0 || mp->thr_x_den > 4096 || mp->thr_y_den == 0 || mp->thr_y_den > 4096 ||
+      mp->thr_x_num > (1u << 20) || mp->thr_y_num > (1u << 20) || mp->ndf == 0 || mp->ndf > 16)
+    return fail(h, CBM_ERR_INVALID_ARG, "msd params: need 0 < den <= 4096, num <= 2^20, 1 <= ndf <= 16");
+  if (n_hits >= (1ull << 32)) return fail(h, CBM_ERR_CAPACITY, "n_hits must be < 2^32");
+  if (n_events && (!d_off || !d_n_passing || !d_accept || (n_hits && (!d_x || !d_y))))
+    return fail(h, CBM_ERR_INVALID_ARG, "device pointers must not be NULL");
+  if (n_events == 0) return CBM_OK;
+  MsdDev d;
+  d.L = h->p.L; d.first_layer = 3 * st;
+  d.z0 = h->p.z[3 * st]; d.z1 = h->p.z[3 * st + 1]; d.z2 = h->p.z[3 * st + 2];
+  d.num_x = mp->thr_x_num; d.den_x = mp->thr_x_den; d.num_y = mp->thr_y_num; d.den_y = mp->thr_y_den;
+  d.ndf = mp->ndf; d.min_triplets = mp->min_triplets;
+  // delta = floor(sqrt(thr * ndf)) + 1 in 10-um units: every residual of a passing triplet is smaller
+  auto delta = [&](uint32_t num, uint32_t den) {
+    const long double v = (long double)num * 1000000.0L * (long double)mp->ndf / (long double)den;
+    return (int64_t)std::floor(std::sqrt(v)) + 2;  // + 1 for the bound, + 1 against the rounding of sqrt
+  };
+  d.pre_x = delta(d.num_x, d.den_x) * ((int64_t)d.z0 + d.z1);
+  d.pre_y = delta(d.num_y, d.den_y) * ((int64_t)d.z0 + d.z1);
+  CBM_CUDA(h, cudaSetDevice(h->cfg.device));
+  msd_kernel<<<(n_events + kMsdWarps - 1) / kMsdWarps, 32 * kMsdWarps, 0, (cudaStream_t)stream>>>(
+      d, d_x, d_y, d_off, n_events, (uint32_t)n_hits, d_n_passing, d_accept);
+  CBM_CUDA(h, cudaGetLastError());
+  return CBM_OK;
 }
 
 int cbm_trigger_get_stats(cbm_trigger_t* h, uint32_t slot, cbm_trigger_stats_t* stats) {
