@@ -27,7 +27,7 @@ using namespace cbm;
 // team classes: warps per team, fullest layer admitted, coarse cells per axis the shared-memory tables hold,
 // middle hits per station kept in shared memory, resident CTAs per SM asked of the compiler
 constexpr int kNfH = 64, kNfM = 32;  // fine cells per axis (at most); coarse = half
-constexpr int kWM = 1, kCapM = 128, kNcM = kNfM / 2, kListM = 128, kMinBM = 19;
+constexpr int kWM = 1, kCapM = 128, kNcM = kNfM / 2, kListM = 32, kMinBM = 24;
 constexpr int kWH = 4, kCapH = 448, kNcH = kNfH / 2, kListH = 64, kMinBH = 8;
 constexpr int kWG = 16, kCapG = 4096, kNcG = kNfH / 2, kListG = 512, kMinBG = 1;
 using SmemM = TeamSmem<kWM, kCapM, kNcM, kListM>;
