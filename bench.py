@@ -307,7 +307,7 @@ def run_ours(args, cfg, cid):
     e2e = e2e_packed = None
     if not args.no_e2e:
         e2e = run_e2e(args, cfg, cid, batch, K, W, local_rank, rank, barrier)
-        if not args.no_packed and cfg.chunk_events == 0:
+        if not args.no_packed:
             e2e_packed = run_e2e(args, cfg, cid, batch, K, W, local_rank, rank, barrier, packed=True)
     del dx, dy, doff
 
