@@ -157,6 +157,18 @@ int cbm_trigger_fetch_selected(cbm_trigger_t* h, uint32_t slot, uint32_t* event_
 int cbm_trigger_select_device(cbm_trigger_t* h, uint32_t n_events, const uint8_t* d_accept, uint32_t* d_event_ids,
                               uint32_t* d_n_selected, void* stream);
 
+/* The hits of the selected events as a compact batch (the selected events go
+ * on to full track reconstruction), on caller-owned DEVICE arrays on the caller's stream.  In: the batch
+ * (d_x, d_y, d_off as in cbm_trigger_run_device) and the list from cbm_trigger_select_device (d_event_ids,
+ * *d_n_selected: the count is read on the device, no host synchronisation).  Out, same layout restricted to the
+ * selected events in list order: d_out_off[n_selected*L + 1] (starts at 0; room for n_events*L + 1 uint32),
+ * d_out_x / d_out_y (room for all n_hits int32 in the worst case), *d_out_n_hits (uint64) = hits gathered.
+ * No atomics: the output is unique.  Asynchronous; uses the handle's scratch (stream-ordered calls only). */
+int cbm_trigger_gather_device(cbm_trigger_t* h, uint32_t n_events, const int32_t* d_x, const int32_t* d_y,
+                              const uint32_t* d_off, const uint32_t* d_event_ids, const uint32_t* d_n_selected,
+                              int32_t* d_out_x, int32_t* d_out_y, uint32_t* d_out_off, unsigned long long* d_out_n_hits,
+                              void* stream);
+
 /* The paper's own selection, literally (section 3.2), on caller-owned DEVICE
  * arrays (layout and stream as cbm_trigger_run_device; geometry = the handle's layer_z):
  *   1. all triplets of the trigger station, one hit from each layer

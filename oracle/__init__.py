@@ -201,3 +201,16 @@ def run_msd(par: MsdParams, x, y, off, e_begin=0, e_end=None):
     if rc != 0:
         raise RuntimeError(f"cbm_msd_oracle_run failed: {rc}")
     return npass, ac
+
+
+def gather(x, y, off, n_layers, event_ids):
+    """The hits of the listed events as a batch of the same layout, event by
+    event and layer by layer.  Returns (x, y, off) with off[0] = 0."""
+    xs, ys, o = [], [], [0]
+    for e in np.asarray(event_ids).ravel().tolist():
+        for l in range(n_layers):
+            a, b = int(off[e * n_layers + l]), int(off[e * n_layers + l + 1])
+            xs.extend(np.asarray(x[a:b]).tolist())
+            ys.extend(np.asarray(y[a:b]).tolist())
+            o.append(o[-1] + (b - a))
+    return np.asarray(xs, dtype=np.int32), np.asarray(ys, dtype=np.int32), np.asarray(o, dtype=np.uint32)

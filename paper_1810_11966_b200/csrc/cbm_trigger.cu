@@ -44,6 +44,7 @@ struct Scratch {
   uint32_t* d_list[kNumTeamClasses] = {nullptr, nullptr, nullptr};
   uint32_t* d_spill[kNumTeamClasses] = {nullptr, nullptr, nullptr};  // per CTA: middle-hit lists beyond shared memory
   uint32_t* d_selcnt = nullptr;  // accepted events per block of kSelEvents events (select.cuh)
+  uint32_t* d_hitbase = nullptr; // first hit of every selected event in the gathered batch (select.cuh)
 };
 
 struct ProfEvents {
@@ -202,6 +203,7 @@ int build_params(const cbm_trigger_config_t& c, Params& p, std::string& why) {
 int alloc_scratch(cbm_trigger* h, Scratch& s) {
   CBM_CUDA(h, cudaMalloc(&s.d_ctrl, sizeof(Ctrl)));
   CBM_CUDA(h, cudaMalloc(&s.d_selcnt, ((size_t)h->cfg.max_events / kSelEvents + 1) * sizeof(uint32_t)));
+  CBM_CUDA(h, cudaMalloc(&s.d_hitbase, ((size_t)h->cfg.max_events + 1) * sizeof(uint32_t)));
   const size_t cap[kNumTeamClasses] = {kCapM, kCapH, kCapG};
   for (int c = 0; c < kNumTeamClasses; ++c) {
     CBM_CUDA(h, cudaMalloc(&s.d_list[c], (size_t)h->cfg.max_events * sizeof(uint32_t)));
@@ -212,6 +214,7 @@ int alloc_scratch(cbm_trigger* h, Scratch& s) {
 void free_scratch(Scratch& s) {
   cudaFree(s.d_ctrl);
   cudaFree(s.d_selcnt);
+  cudaFree(s.d_hitbase);
   for (int c = 0; c < kNumTeamClasses; ++c) { cudaFree(s.d_list[c]); cudaFree(s.d_spill[c]); }
   s = Scratch();
 }
@@ -647,6 +650,29 @@ int cbm_trigger_select_device(cbm_trigger_t* h, uint32_t n_events, const uint8_t
   CBM_CUDA(h, cudaSetDevice(h->cfg.device));
   const int nl = launch_compaction(h, h->dev_scr, d_accept, n_events, d_event_ids, d_n_selected, (cudaStream_t)stream);
   return nl < 0 ? nl : CBM_OK;
+}
+
+int cbm_trigger_gather_device(cbm_trigger_t* h, uint32_t n_events, const int32_t* d_x, const int32_t* d_y,
+                              const uint32_t* d_off, const uint32_t* d_event_ids, const uint32_t* d_n_selected,
+                              int32_t* d_out_x, int32_t* d_out_y, uint32_t* d_out_off, unsigned long long* d_out_n_hits,
+                              void* stream) {
+  if (!h) return CBM_ERR_INVALID_ARG;
+  if (n_events > h->cfg.max_events) return fail(h, CBM_ERR_CAPACITY, "n_events %u > max_events %u", n_events, h->cfg.max_events);
+  if (!d_n_selected || !d_out_off || !d_out_n_hits || (n_events && (!d_off || !d_event_ids || !d_x || !d_y || !d_out_x || !d_out_y)))
+    return fail(h, CBM_ERR_INVALID_ARG, "device pointers must not be NULL");
+  static_assert(kGatherEvents == kSelEvents, "the per-block scratch is shared with the selection list");
+  CBM_CUDA(h, cudaSetDevice(h->cfg.device));
+  cudaStream_t st = (cudaStream_t)stream;
+  const uint32_t nb = n_events / kGatherEvents + 1;
+  const Scratch& scr = h->dev_scr;
+  gather_size_kernel<<<nb, kSelThreads, 0, st>>>(d_off, h->p.L, d_event_ids, d_n_selected, scr.d_selcnt);
+  gather_base_kernel<<<nb, kSelThreads, 0, st>>>(d_off, h->p.L, d_event_ids, d_n_selected, scr.d_selcnt, scr.d_hitbase,
+                                                 d_out_off, d_out_n_hits);
+  if (n_events)
+    gather_copy_kernel<<<h->n_sm * 8, kSelThreads, 0, st>>>(d_x, d_y, d_off, h->p.L, d_event_ids, d_n_selected,
+                                                            scr.d_hitbase, d_out_x, d_out_y, d_out_off);
+  CBM_CUDA(h, cudaGetLastError());
+  return CBM_OK;
 }
 
 int cbm_trigger_msd_device(cbm_trigger_t* h, const cbm_trigger_msd_params_t* mp, uint32_t n_events, uint64_t n_hits,

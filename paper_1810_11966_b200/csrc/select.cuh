@@ -84,4 +84,83 @@ __global__ void __launch_bounds__(kSelThreads)
   if (blockIdx.x == gridDim.x - 1 && threadIdx.x == 0) *n_selected = base_sh + total;
 }
 
+// ---------------------------------------------------------------------------------------------- gather
+// The hits of the selected events as a compact batch of the same layout (what the
+// next trigger level, full track reconstruction, reads).  Three steps, no atomics, so the
+// output is unique: sizes of the selected events and their per-block sums; exclusive prefix of the sizes (every
+// block adds the sums of the blocks before it); one CTA per selected event copies its hits and writes its
+// offsets rebased to the new batch.
+constexpr int kGatherPerThread = 16;
+constexpr int kGatherEvents = kSelThreads * kGatherPerThread;
+
+__device__ __forceinline__ uint32_t gather_event_size(const uint32_t* __restrict__ off, uint32_t L, uint32_t e) {
+  return __ldg(off + (size_t)e * L + L) - __ldg(off + (size_t)e * L);
+}
+
+__global__ void __launch_bounds__(kSelThreads)
+    gather_size_kernel(const uint32_t* __restrict__ off, uint32_t L, const uint32_t* __restrict__ ids,
+                       const uint32_t* __restrict__ n_selected, uint32_t* __restrict__ block_sum) {
+  __shared__ uint32_t warp_sums[kSelThreads / 32];
+  const uint32_t n = *n_selected;
+  const uint32_t first = (blockIdx.x * kSelThreads + threadIdx.x) * kGatherPerThread;
+  uint32_t sum = 0;
+  for (uint32_t i = first; i < min(first + kGatherPerThread, n); ++i) sum += gather_event_size(off, L, __ldg(ids + i));
+  uint32_t total;
+  sel_block_exclusive_scan(sum, warp_sums, &total);
+  if (threadIdx.x == 0) block_sum[blockIdx.x] = total;
+}
+
+__global__ void __launch_bounds__(kSelThreads)
+    gather_base_kernel(const uint32_t* __restrict__ off, uint32_t L, const uint32_t* __restrict__ ids,
+                       const uint32_t* __restrict__ n_selected, const uint32_t* __restrict__ block_sum,
+                       uint32_t* __restrict__ hit_base, uint32_t* __restrict__ out_off, unsigned long long* __restrict__ out_n_hits) {
+  __shared__ uint32_t warp_sums[kSelThreads / 32];
+  __shared__ uint32_t base_sh;
+  const uint32_t n = *n_selected;
+  uint32_t part = 0;
+  for (uint32_t b = threadIdx.x; b < blockIdx.x; b += kSelThreads) part += block_sum[b];
+  uint32_t before;
+  sel_block_exclusive_scan(part, warp_sums, &before);
+  if (threadIdx.x == 0) base_sh = before;
+  __syncthreads();
+  const uint32_t first = (blockIdx.x * kSelThreads + threadIdx.x) * kGatherPerThread;
+  uint32_t sz[kGatherPerThread], sum = 0;
+#pragma unroll
+  for (int k = 0; k < kGatherPerThread; ++k) {
+    sz[k] = first + k < n ? gather_event_size(off, L, __ldg(ids + first + k)) : 0u;
+    sum += sz[k];
+  }
+  uint32_t total;
+  uint32_t pos = base_sh + sel_block_exclusive_scan(sum, warp_sums, &total);
+#pragma unroll
+  for (int k = 0; k < kGatherPerThread; ++k) {
+    if (first + k < n) hit_base[first + k] = pos;
+    pos += sz[k];
+  }
+  // the block holding the end of the list closes the offset table and reports the number of hits
+  const uint32_t last_block = n ? (n - 1) / kGatherEvents : 0u;
+  if (blockIdx.x == last_block && threadIdx.x == 0) {
+    out_off[(size_t)n * L] = base_sh + total;
+    *out_n_hits = base_sh + total;
+  }
+}
+
+// one CTA per selected event (grid-stride)
+__global__ void __launch_bounds__(kSelThreads)
+    gather_copy_kernel(const int32_t* __restrict__ x, const int32_t* __restrict__ y, const uint32_t* __restrict__ off,
+                       uint32_t L, const uint32_t* __restrict__ ids, const uint32_t* __restrict__ n_selected,
+                       const uint32_t* __restrict__ hit_base, int32_t* __restrict__ out_x, int32_t* __restrict__ out_y,
+                       uint32_t* __restrict__ out_off) {
+  const uint32_t n = *n_selected;
+  for (uint32_t i = blockIdx.x; i < n; i += gridDim.x) {
+    const uint32_t e = __ldg(ids + i), dst = hit_base[i];
+    const uint32_t src = __ldg(off + (size_t)e * L), end = __ldg(off + (size_t)e * L + L);
+    for (uint32_t l = threadIdx.x; l < L; l += kSelThreads) out_off[(size_t)i * L + l] = dst + (__ldg(off + (size_t)e * L + l) - src);
+    for (uint32_t k = threadIdx.x; k < end - src; k += kSelThreads) {
+      out_x[dst + k] = __ldg(x + src + k);
+      out_y[dst + k] = __ldg(y + src + k);
+    }
+  }
+}
+
 }  // namespace cbm

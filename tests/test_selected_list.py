@@ -108,3 +108,67 @@ def test_select_device_on_arbitrary_flags(n):
             want = oracle.selected(a[shift:])
             assert int(d_n.item()) == want.size
             assert np.array_equal(d_ids.cpu().numpy().view(np.uint32)[:want.size], want)
+
+
+# ------------------------------------------------------------------------------------------------ gather
+def test_oracle_gather_hand_case_and_identity():
+    # 2 layers per "event" for brevity (the routine only needs the layer count): event 0: [1,2 | 3], event 1: [ | 4,5],
+    # event 2: [6 | ]
+    x = np.array([1, 2, 3, 4, 5, 6], np.int32)
+    y = -x
+    off = np.array([0, 2, 3, 3, 5, 6, 6], np.uint32)
+    gx, gy, go = oracle.gather(x, y, off, 2, [2, 0])
+    assert gx.tolist() == [6, 1, 2, 3] and gy.tolist() == [-6, -1, -2, -3] and go.tolist() == [0, 1, 1, 3, 4]
+    gx, gy, go = oracle.gather(x, y, off, 2, [])
+    assert gx.size == 0 and go.tolist() == [0]
+    # every event in order gives the batch back
+    cfg = W.CONFIGS[0]
+    b = W.generate(cfg, n_events=50)
+    gx, gy, go = oracle.gather(b.x, b.y, b.off, cfg.n_layers, np.arange(50))
+    assert np.array_equal(gx, b.x) and np.array_equal(gy, b.y) and np.array_equal(go, b.off)
+    # the gathered batch of the selected events gives the selected events' results
+    g = oracle.geometry(cfg.layer_z, cfg.win_in, cfg.win_link, cfg.min_candidates)
+    nt, nc, ac = oracle.run(g, b.x, b.y, b.off)
+    ids = oracle.selected(ac)
+    gx, gy, go = oracle.gather(b.x, b.y, b.off, cfg.n_layers, ids)
+    nt2, nc2, ac2 = oracle.run(g, gx, gy, go)
+    assert np.array_equal(nt2, nt[ids]) and np.array_equal(nc2, nc[ids]) and ac2.all()
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("cid,n,minc", [(0, 1000, 2), (3, 9000, 2), (1, 700, 0), (2, 600, 2), (0, 300, 0xFFFFFFFF)])
+def test_gather_device_matches_oracle(cid, n, minc):
+    """run_device -> select_device -> gather_device on device arrays, against oracle.selected / oracle.gather."""
+    import torch
+    from paper_1810_11966_b200 import binding as K
+    from tests.helpers import oracle_mt
+    cfg = W.CONFIGS[cid]
+    b = W.generate(cfg, n_events=n)
+    g = oracle.geometry(cfg.layer_z, cfg.win_in, cfg.win_link, minc)
+    _, _, oac = oracle_mt(g, b.x, b.y, b.off)
+    want_ids = oracle.selected(oac)
+    wx, wy, wo = oracle.gather(b.x, b.y, b.off, cfg.n_layers, want_ids)
+    S, L = cfg.n_stations, cfg.n_layers
+    with K.Trigger(cfg.layer_z, n, b.n_hits, win_in=cfg.win_in, win_link=cfg.win_link, min_candidates=minc, n_slots=0) as trig:
+        pad = lambda a: torch.from_numpy(np.concatenate([a.view(np.int32), np.zeros(8, np.int32)])).cuda()
+        dx, dy = pad(b.x), pad(b.y)
+        do = torch.from_numpy(b.off.view(np.int32)).cuda()
+        dnt = torch.zeros(n * S, dtype=torch.int32, device="cuda")
+        dnc = torch.zeros(n, dtype=torch.int32, device="cuda")
+        dac = torch.zeros(n, dtype=torch.uint8, device="cuda")
+        dids = torch.zeros(n, dtype=torch.int32, device="cuda")
+        dn = torch.zeros(1, dtype=torch.int32, device="cuda")
+        ox = torch.full((b.n_hits + 1,), 77, dtype=torch.int32, device="cuda")
+        oy = torch.full((b.n_hits + 1,), 77, dtype=torch.int32, device="cuda")
+        oo = torch.full((n * L + 1,), -1, dtype=torch.int32, device="cuda")
+        on = torch.zeros(1, dtype=torch.int64, device="cuda")
+        trig.run_device(n, b.n_hits, dx, dy, do, dnt, dnc, dac)
+        trig.select_device(n, dac, dids, dn)
+        trig.gather_device(n, dx, dy, do, dids, dn, ox, oy, oo, on)
+        torch.cuda.synchronize()
+        ns, nh = int(dn.item()), int(on.item())
+        assert ns == want_ids.size and nh == wx.size
+        assert np.array_equal(dids.cpu().numpy().view(np.uint32)[:ns], want_ids)
+        assert np.array_equal(oo.cpu().numpy().view(np.uint32)[:ns * L + 1], wo)
+        assert np.array_equal(ox.cpu().numpy()[:nh], wx) and np.array_equal(oy.cpu().numpy()[:nh], wy)
+        assert int(ox[nh].item()) == 77  # nothing written past the end
