@@ -326,10 +326,11 @@ def run_ours(args, cfg, cid):
 
     # ---- roofline of the dominant kernel: algorithmic bytes of the events it processes / its mean launch time
     acct = class_accounting(batch.off, S, K.TINY_MAX_LAYER_DEFAULT, K.TINY_MAX_TOTAL, K.CLASS_CAPS)
-    kmean = ktimes.mean(axis=0) if len(ktimes) else np.zeros(4)
-    # the tile kernel also reads every event's offsets (classification) and writes the tiny events' results
+    kmean = ktimes.mean(axis=0) if len(ktimes) else np.zeros(K.N_KERNELS)
+    # kernels: classify (reads every event's offsets), tile, team_M, team_H, team_G, team_X (events handed on)
+    zero = {"events": 0, "hits": 0, "bytes": 0}
+    acct = [{"events": E, "hits": 0, "bytes": 4 * (E * 3 * S + 1)}] + acct + [zero]
     kbytes = [a["bytes"] for a in acct]
-    kbytes[0] += sum(a["events"] for a in acct[1:]) * 4 * 3 * S
     # dominant kernel = the one that moves the most algorithmic bytes.  (The three class kernels run side by
     # side on their own streams after the tile kernel, so the event-to-event time of a small class also counts
     # its wait for SMs; the times of the tile kernel and of the dominant class kernel are their own.)
@@ -350,7 +351,7 @@ def run_ours(args, cfg, cid):
                    if B_alg > 200e6 else "inputs smaller than L2: L2-resident between steps", "parallelism": f"replicas x{world}"},
         "hits_per_second": hits_all * args.steps / (ms_total_max * 1e-3),
         "vs_10MHz": value / CBM_INTERACTION_RATE_HZ,
-        "gpu_launches": 4 * args.steps,
+        "gpu_launches": K.N_KERNELS * args.steps,
         "kernels": {name: {"ms": float(kmean[i]), "events": acct[i]["events"], "hits": acct[i]["hits"],
                            "algorithmic_bytes": kbytes[i]} for i, name in enumerate(K.KERNEL_NAMES)},
         "classes": stats["n_class"], "accepted_events": n_accept, "events_with_candidates": n_cand_events,

@@ -45,7 +45,7 @@ extern "C" {
 #define CBM_TRIGGER_MAX_LAYERS 24
 #define CBM_TRIGGER_MAX_HITS_PER_LAYER 4096
 #define CBM_TRIGGER_MAX_SLOTS 4
-#define CBM_TRIGGER_N_KERNELS 4 /* tile, team_M, team_H, team_G (see cbm_trigger_stats_t) */
+#define CBM_TRIGGER_N_KERNELS 6 /* classify, tile, team_M, team_H, team_G, team_X (see cbm_trigger_stats_t) */
 #define CBM_TRIGGER_PROFILE_RING 32 /* run_device calls whose per-kernel times are kept (CBM_FLAG_PROFILE) */
 
 enum {
@@ -73,7 +73,6 @@ typedef struct {
   uint32_t n_slots;                    /* 0..4 slots of (pinned host + device) buffers; 2 = double buffering.
                                           0: only cbm_trigger_run_device() is usable (caller owns all buffers) */
   int32_t  device;                     /* CUDA ordinal */
-  uint32_t slope_range_milli;          /* ignored (kept for ABI layout): the slope grid is cyclic and needs no range */
   uint32_t tiny_max_layer_hits;        /* tuning: events whose fullest layer holds <= this many hits (and that fit
                                           the tile) take the thread-per-station path. 0 = default (24); max 32 */
   uint32_t flags;                      /* CBM_FLAG_* */
@@ -82,16 +81,21 @@ typedef struct {
 #define CBM_FLAG_PROFILE 1u      /* record CUDA events around every kernel (cbm_trigger_get_stats: kernel_ms) */
 #define CBM_FLAG_NO_TINY_PATH 2u /* tuning/testing: route every event through the team kernels */
 #define CBM_FLAG_PACKED_INPUT 4u /* the slots take the packed wire format XY20 (cbm_trigger_upload_events_packed) */
+#define CBM_FLAG_SERIAL 8u       /* measuring: launch the kernels of a run one after the other on one stream instead of
+                                    side by side, so that kernel_ms are kernel times (results are identical) */
 
 typedef struct {
   uint32_t struct_size;
   uint32_t n_events;
   uint64_t n_hits;
   uint32_t n_class[4];     /* events handled by: [0] tile kernel (tiny), [1] team_M, [2] team_H, [3] team_G */
+  uint32_t n_redone;       /* events one of those kernels handed on (a shared-memory table overflowed); redone by team_X */
   uint32_t n_invalid;      /* events rejected on the device (bad offsets / layer too full); their outputs are 0 */
   uint32_t first_invalid;  /* smallest such event index, 0xFFFFFFFF if none */
   uint32_t n_launches;     /* kernels launched by the last run of this slot */
-  float    kernel_ms[CBM_TRIGGER_N_KERNELS]; /* CBM_FLAG_PROFILE only: device time of each kernel, else 0 */
+  float    kernel_ms[CBM_TRIGGER_N_KERNELS]; /* CBM_FLAG_PROFILE only: device time of classify, tile, team_M, team_H,
+                                                 team_G, team_X (CUDA events on the stream of each), else 0.  Without
+                                                 CBM_FLAG_SERIAL the kernels share the GPU, so a time includes waiting */
   float    h2d_ms, d2h_ms; /* CBM_FLAG_PROFILE only */
 } cbm_trigger_stats_t;
 

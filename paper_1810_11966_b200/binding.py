@@ -15,10 +15,10 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libcbmtrigger.so")
 
 MAX_LAYERS = 24
-N_KERNELS = 4
-KERNEL_NAMES = ("tile_kernel", "team_kernel_M", "team_kernel_H", "team_kernel_G")
+N_KERNELS = 6
+KERNEL_NAMES = ("classify_kernel", "tile_kernel", "team_kernel_M", "team_kernel_H", "team_kernel_G", "team_kernel_X")
 CBM_OK, CBM_ERR_INVALID_ARG, CBM_ERR_RANGE, CBM_ERR_CAPACITY, CBM_ERR_STATE, CBM_ERR_CUDA = 0, -1, -2, -3, -4, -5
-CBM_FLAG_PROFILE, CBM_FLAG_NO_TINY_PATH, CBM_FLAG_PACKED_INPUT = 1, 2, 4
+CBM_FLAG_PROFILE, CBM_FLAG_NO_TINY_PATH, CBM_FLAG_PACKED_INPUT, CBM_FLAG_SERIAL = 1, 2, 4, 8
 EXPORTS = (
     "cbm_trigger_create", "cbm_trigger_destroy", "cbm_trigger_host_buffers", "cbm_trigger_upload_events",
     "cbm_trigger_run", "cbm_trigger_fetch_results", "cbm_trigger_run_device", "cbm_trigger_device_status",
@@ -45,7 +45,6 @@ class Config(ctypes.Structure):
         ("max_hits_per_layer", ctypes.c_uint32),
         ("n_slots", ctypes.c_uint32),
         ("device", ctypes.c_int32),
-        ("slope_range_milli", ctypes.c_uint32),
         ("tiny_max_layer_hits", ctypes.c_uint32),
         ("flags", ctypes.c_uint32),
     ]
@@ -57,6 +56,7 @@ class Stats(ctypes.Structure):
         ("n_events", ctypes.c_uint32),
         ("n_hits", ctypes.c_uint64),
         ("n_class", ctypes.c_uint32 * 4),
+        ("n_redone", ctypes.c_uint32),
         ("n_invalid", ctypes.c_uint32),
         ("first_invalid", ctypes.c_uint32),
         ("n_launches", ctypes.c_uint32),
@@ -65,7 +65,7 @@ class Stats(ctypes.Structure):
     ]
 
     def as_dict(self):
-        return {"n_events": self.n_events, "n_hits": self.n_hits, "n_class": list(self.n_class),
+        return {"n_events": self.n_events, "n_hits": self.n_hits, "n_class": list(self.n_class), "n_redone": self.n_redone,
                 "n_invalid": self.n_invalid, "first_invalid": self.first_invalid, "n_launches": self.n_launches,
                 "kernel_ms": [float(v) for v in self.kernel_ms], "h2d_ms": float(self.h2d_ms),
                 "d2h_ms": float(self.d2h_ms)}
@@ -151,7 +151,7 @@ def load_library():
 
 
 def make_config(layer_z, max_events, max_hits, win_in=(1, 100), win_link=(2, 100), min_candidates=2,
-                max_hits_per_layer=4096, n_slots=2, device=0, slope_range_milli=0, tiny_max_layer_hits=0,
+                max_hits_per_layer=4096, n_slots=2, device=0, tiny_max_layer_hits=0,
                 flags=0) -> Config:
     c = Config()
     c.struct_size = ctypes.sizeof(Config)
@@ -164,7 +164,7 @@ def make_config(layer_z, max_events, max_hits, win_in=(1, 100), win_link=(2, 100
     c.max_events, c.max_hits = int(max_events), int(max_hits)
     c.max_hits_per_layer = max_hits_per_layer
     c.n_slots, c.device = n_slots, device
-    c.slope_range_milli, c.tiny_max_layer_hits, c.flags = slope_range_milli, tiny_max_layer_hits, flags
+    c.tiny_max_layer_hits, c.flags = tiny_max_layer_hits, flags
     return c
 
 

@@ -15,7 +15,9 @@
 #include <string>
 
 #include "../../include/cbm_trigger.h"
-#include "kernels.cuh"
+#include "classify.cuh"
+#include "tile.cuh"
+#include "team.cuh"
 #include "select.cuh"
 #include "wire.cuh"
 #include "msd.cuh"
@@ -24,25 +26,27 @@ namespace {
 
 using namespace cbm;
 
-// team classes: warps per team, fullest layer admitted, coarse cells per axis the shared-memory tables hold,
-// middle hits per station kept in shared memory, resident CTAs per SM asked of the compiler
-constexpr int kNfH = 64, kNfM = 32;  // fine cells per axis (at most); coarse = half
-constexpr int kWM = 1, kCapM = 128, kNcM = kNfM / 2, kListM = 32, kMinBM = 24;
-constexpr int kWH = 4, kCapH = 448, kNcH = kNfH / 2, kListH = 64, kMinBH = 8;
-constexpr int kWG = 16, kCapG = 4096, kNcG = kNfH / 2, kListG = 512, kMinBG = 1;
-using SmemM = TeamSmem<kWM, kCapM, kNcM, kListM>;
-using SmemH = TeamSmem<kWH, kCapH, kNcH, kListH>;
-using SmemG = TeamSmem<kWG, kCapG, kNcG, kListG>;
-#define TEAM_KERNEL_M team_kernel<kWM, kCapM, kNcM, kListM, kClsM, kMinBM, true>
-#define TEAM_KERNEL_H team_kernel<kWH, kCapH, kNcH, kListH, kClsH, kMinBH, true>
-#define TEAM_KERNEL_G team_kernel<kWG, kCapG, kNcG, kListG, kClsG, kMinBG, false>
+// team classes (team.cuh): warps per team, fullest layer admitted, kept middle hits, band width (log2 cell
+// columns), kept hits per band, overflow band, middle hits with triplets per station, resident CTAs per SM
+using SmemM = TeamSmem<1, 128, 64, 3, 8, 32, 32>;
+using SmemH = TeamSmem<4, 448, 192, 2, 16, 64, 48>;
+using SmemG = TeamSmem<16, 4096, 4096, 0, 32, 4096, 256>;
+constexpr int kCapM = SmemM::CAP, kCapH = SmemH::CAP, kCapG = SmemG::CAP;
+constexpr int kMinBM = 24, kMinBH = 10, kMinBG = 1;
+#define TEAM_KERNEL_M team_kernel<SmemM, kClsM, kMinBM, false, true>
+#define TEAM_KERNEL_H team_kernel<SmemH, kClsH, kMinBH, false, true>
+#define TEAM_KERNEL_G team_kernel<SmemG, kClsG, kMinBG, true, false>
+#define TEAM_KERNEL_X team_kernel<SmemG, kClsX, kMinBG, true, false>
+// kernels of one run, in the order of cbm_trigger_stats_t::kernel_ms
+enum { kKClassify = 0, kKTile = 1, kKTeamM = 2, kKTeamH = 3, kKTeamG = 4, kKTeamX = 5 };
+static_assert(CBM_TRIGGER_N_KERNELS == 6, "kernel_ms layout");
 
 enum SlotState { kEmpty = 0, kUploaded = 1, kRunning = 2 };
 
 struct Scratch {
   Ctrl* d_ctrl = nullptr;
-  uint32_t* d_list[kNumTeamClasses] = {nullptr, nullptr, nullptr};
-  uint32_t* d_spill[kNumTeamClasses] = {nullptr, nullptr, nullptr};  // per CTA: middle-hit lists beyond shared memory
+  uint32_t* d_list[kNumLists] = {nullptr, nullptr, nullptr, nullptr};  // M, H, G, X
+  uint32_t* d_spill[2] = {nullptr, nullptr};  // class G, list X; per CTA: middle-hit lists beyond shared memory
   uint32_t* d_selcnt = nullptr;  // accepted events per block of kSelEvents events (select.cuh)
   uint32_t* d_hitbase = nullptr; // first hit of every selected event in the gathered batch (select.cuh)
 };
@@ -84,7 +88,7 @@ struct cbm_trigger {
   cbm_trigger_config_t cfg;
   Params p;
   int n_sm = 0;
-  int grid[kNumTeamClasses] = {0, 0, 0};
+  int grid[kNumLists] = {0, 0, 0, 0};
   Slot slot[CBM_TRIGGER_MAX_SLOTS];
   Scratch dev_scr;          // scratch of cbm_trigger_run_device
   Ctrl* h_dev_ctrl = nullptr;
@@ -93,8 +97,8 @@ struct cbm_trigger {
   uint32_t dev_n_events = 0;
   uint64_t dev_n_hits = 0;
   cudaStream_t st_h2d = nullptr, st_run = nullptr, st_d2h = nullptr;
-  cudaStream_t st_side[2] = {nullptr, nullptr};  // classes M and G run beside class H (after the tile kernel)
-  cudaEvent_t ev_fork = nullptr, ev_join[2] = {nullptr, nullptr};
+  cudaStream_t st_side[3] = {nullptr, nullptr, nullptr};  // tile, M and G run beside class H (after classify)
+  cudaEvent_t ev_fork = nullptr, ev_join[3] = {nullptr, nullptr, nullptr};
   std::string err;
 };
 
@@ -170,26 +174,27 @@ int build_params(const cbm_trigger_config_t& c, Params& p, std::string& why) {
   // Slope keys: key = floor(x*M_l/2^32), M_l = round(2^32*K/z_l) < 2^31.
   // For any int32 x: |x*M_l/2^32 - K*x/z_l| <= 2^31 * 0.5/2^32 = 0.25, floor loses < 1  =>  |key - K*x/z_l| < 1.25.
   // Two hits with |x_h/z_A - x_g/z_B| <= w therefore have |key_h - key_g| < w*K + 2.5 <= R := ceil(w*K) + 3.
-  // Grid: fine cell = floor(key / 2^fsh) mod nf (cyclic, so no slope range has to be covered), 2^fsh >= R:
-  // compatible hits lie in fine cells at most one apart; a coarse cell = two fine cells >= 2R, so a window
-  // touches at most 2 x 2 coarse cells.  K is chosen so that the fine cell is as narrow as the window allows.
+  // K is the largest scale with R <= 254 (and K < z_min/2): then the packed 16-bit test below is as sharp as the
+  // window itself.  Filter cell = floor(key / 2^cell_sh) mod 64 with 2^cell_sh >= R: hits that are pairwise
+  // compatible span at most two adjacent cells per axis (cyclic grid: no slope range has to be covered).
   const double w = (double)c.win_in_num / (double)c.win_in_den;
   const double Kmax = 0.499 * (double)p.z[0];
-  int fsh = 2, R = 3;
-  double K = 0, best = 1e300;
-  for (int sh = 2; sh <= 14; ++sh) {
-    const double two = std::ldexp(1.0, sh);
-    const double k = w > 0 ? std::min(Kmax, (two - 3.0) / w * (1.0 - 1e-9)) : Kmax;
-    if (k <= 0) continue;
-    const int r = (int)std::ceil(w * k) + 3;
-    if (r <= (1 << sh) && two / k < best) { best = two / k; fsh = sh; K = k; R = r; }
-  }
-  if (K <= 0) { why = "internal: no slope key scale"; return CBM_ERR_INVALID_ARG; }
+  const double K = w > 0 ? std::min(Kmax, (254.0 - 3.0) / w * (1.0 - 1e-9)) : Kmax;
+  if (!(K > 0)) { why = "internal: no slope key scale"; return CBM_ERR_INVALID_ARG; }
+  const int R = (int)std::ceil(w * K) + 3;
+  if (R < 3 || R > 254) { why = "internal: slope key window out of range"; return CBM_ERR_INVALID_ARG; }
   p.key_R = R;
-  p.cls_nf[kClsH] = p.cls_nf[kClsG] = (uint32_t)kNfH;
-  p.cls_fsh[kClsH] = p.cls_fsh[kClsG] = fsh;
-  p.cls_nf[kClsM] = (uint32_t)kNfM;  // fewer hits per layer: cells twice as wide
-  p.cls_fsh[kClsM] = fsh + 1;
+  int sh = 2;
+  while ((1 << sh) < R) ++sh;
+  p.cell_sh = sh;
+  // Packed test: P = (kx mod 2^16) | (ky mod 2^16) << 16.  With key_add = R | (R+1) << 16 the low half of
+  // P_a + key_add - P_b is (dkx + R) mod 2^16 in [0, 2R] and the high half is (dky + R + 1 + carry) mod 2^16,
+  // carry in {-1, 0, 1}, in [0, 2R+2], whenever |dkx|, |dky| <= R: both halves are below 2^m >= 2R + 3.
+  int m = 3;
+  while ((1 << m) < 2 * R + 3) ++m;
+  const uint32_t half = 0xFFFFu & ~((1u << m) - 1u);
+  p.key_mask = half | (half << 16);
+  p.key_add = (uint32_t)R | ((uint32_t)(R + 1) << 16);
   for (uint32_t l = 0; l < p.L; ++l) {
     const double m = std::ldexp(K, 32) / (double)p.z[l];
     const long long mi = llround(m);
@@ -204,18 +209,18 @@ int alloc_scratch(cbm_trigger* h, Scratch& s) {
   CBM_CUDA(h, cudaMalloc(&s.d_ctrl, sizeof(Ctrl)));
   CBM_CUDA(h, cudaMalloc(&s.d_selcnt, ((size_t)h->cfg.max_events / kSelEvents + 1) * sizeof(uint32_t)));
   CBM_CUDA(h, cudaMalloc(&s.d_hitbase, ((size_t)h->cfg.max_events + 1) * sizeof(uint32_t)));
-  const size_t cap[kNumTeamClasses] = {kCapM, kCapH, kCapG};
-  for (int c = 0; c < kNumTeamClasses; ++c) {
-    CBM_CUDA(h, cudaMalloc(&s.d_list[c], (size_t)h->cfg.max_events * sizeof(uint32_t)));
-    CBM_CUDA(h, cudaMalloc(&s.d_spill[c], (size_t)h->grid[c] * 6 * cap[c] * sizeof(uint32_t)));
-  }
+  for (int c = 0; c < kNumLists; ++c) CBM_CUDA(h, cudaMalloc(&s.d_list[c], (size_t)h->cfg.max_events * sizeof(uint32_t)));
+  CBM_CUDA(h, cudaMalloc(&s.d_spill[0], (size_t)h->grid[kClsG] * 6 * kCapG * sizeof(uint32_t)));
+  CBM_CUDA(h, cudaMalloc(&s.d_spill[1], (size_t)h->grid[kClsX] * 6 * kCapG * sizeof(uint32_t)));
   return CBM_OK;
 }
 void free_scratch(Scratch& s) {
   cudaFree(s.d_ctrl);
   cudaFree(s.d_selcnt);
   cudaFree(s.d_hitbase);
-  for (int c = 0; c < kNumTeamClasses; ++c) { cudaFree(s.d_list[c]); cudaFree(s.d_spill[c]); }
+  for (int c = 0; c < kNumLists; ++c) cudaFree(s.d_list[c]);
+  cudaFree(s.d_spill[0]);
+  cudaFree(s.d_spill[1]);
   s = Scratch();
 }
 int make_prof(cbm_trigger* h, ProfEvents& pe) {
@@ -283,7 +288,11 @@ void free_slot(Slot& s) {
 }
 
 // ---------------------------------------------------------------------------------------------- launches
-// a3..a8 on one stream.  Returns the number of kernels launched (0 on an empty batch), < 0 on error.
+// a3..a8.  classify_kernel on the caller's stream; then the tile kernel and the class kernels M, G on side
+// streams beside class H on the caller's stream (disjoint events), joined before the list-X kernel, which
+// redoes the few events another kernel handed on.  CBM_FLAG_SERIAL: everything on the caller's stream, one
+// kernel after the other (per-kernel times that are kernel times).
+// Returns the number of kernels launched (0 on an empty batch), < 0 on error.
 int launch_selection(cbm_trigger* h, const Scratch& scr, const int32_t* d_x, const int32_t* d_y, const uint32_t* d_off,
                      uint32_t n_events, uint64_t n_hits, uint32_t* d_nt, uint32_t* d_nc, uint8_t* d_ac,
                      cudaStream_t st, ProfEvents* prof) {
@@ -291,38 +300,57 @@ int launch_selection(cbm_trigger* h, const Scratch& scr, const int32_t* d_x, con
   CBM_CUDA(h, cudaMemsetAsync(scr.d_ctrl, 0, sizeof(Ctrl), st));
   if (prof) prof->valid = false;
   if (n_events == 0) return 0;
-  if (prof) CBM_CUDA(h, cudaEventRecord(prof->k[0], st));
-  const uint32_t n_tiles = (n_events + kTileEvents - 1) / kTileEvents;
-  if (p.S <= 4)  // tables sized for 4 stations: more resident CTAs
-    tile_kernel<4><<<n_tiles, kTileEvents * p.S, 0, st>>>(p, d_x, d_y, d_off, n_events, (uint32_t)n_hits, d_nt, d_nc, d_ac,
-                                                          scr.d_ctrl, scr.d_list[kClsM], scr.d_list[kClsH], scr.d_list[kClsG]);
-  else
-    tile_kernel<kMaxStations><<<n_tiles, kTileEvents * p.S, 0, st>>>(p, d_x, d_y, d_off, n_events, (uint32_t)n_hits, d_nt, d_nc, d_ac,
-                                                                     scr.d_ctrl, scr.d_list[kClsM], scr.d_list[kClsH], scr.d_list[kClsG]);
-  if (prof) CBM_CUDA(h, cudaEventRecord(prof->k[1], st));
-  // The three class kernels are independent (disjoint events): M and G on side streams, H on the caller's.
-  // M and G are launched first: most of their persistent CTAs find an empty list and leave at once.
-  CBM_CUDA(h, cudaEventRecord(h->ev_fork, st));
-  CBM_CUDA(h, cudaStreamWaitEvent(h->st_side[0], h->ev_fork, 0));
-  CBM_CUDA(h, cudaStreamWaitEvent(h->st_side[1], h->ev_fork, 0));
-  if (prof) CBM_CUDA(h, cudaEventRecord(prof->k[2], h->st_side[0]));
-  TEAM_KERNEL_M<<<h->grid[kClsM], 32 * kWM, 0, h->st_side[0]>>>(
-      p, d_x, d_y, d_off, d_nt, d_nc, d_ac, scr.d_ctrl, scr.d_list[kClsM], scr.d_spill[kClsM]);
-  if (prof) CBM_CUDA(h, cudaEventRecord(prof->k[3], h->st_side[0]));
-  CBM_CUDA(h, cudaEventRecord(h->ev_join[0], h->st_side[0]));
-  if (prof) CBM_CUDA(h, cudaEventRecord(prof->k[6], h->st_side[1]));
-  TEAM_KERNEL_G<<<h->grid[kClsG], 32 * kWG, sizeof(SmemG), h->st_side[1]>>>(
-      p, d_x, d_y, d_off, d_nt, d_nc, d_ac, scr.d_ctrl, scr.d_list[kClsG], scr.d_spill[kClsG]);
-  if (prof) CBM_CUDA(h, cudaEventRecord(prof->k[7], h->st_side[1]));
-  CBM_CUDA(h, cudaEventRecord(h->ev_join[1], h->st_side[1]));
-  if (prof) CBM_CUDA(h, cudaEventRecord(prof->k[4], st));
-  TEAM_KERNEL_H<<<h->grid[kClsH], 32 * kWH, 0, st>>>(
-      p, d_x, d_y, d_off, d_nt, d_nc, d_ac, scr.d_ctrl, scr.d_list[kClsH], scr.d_spill[kClsH]);
-  if (prof) { CBM_CUDA(h, cudaEventRecord(prof->k[5], st)); prof->valid = true; }
-  CBM_CUDA(h, cudaStreamWaitEvent(st, h->ev_join[0], 0));
-  CBM_CUDA(h, cudaStreamWaitEvent(st, h->ev_join[1], 0));
+  const bool serial = h->cfg.flags & CBM_FLAG_SERIAL;
+  cudaStream_t s_tile = serial ? st : h->st_side[2], s_m = serial ? st : h->st_side[0], s_g = serial ? st : h->st_side[1];
+  auto rec = [&](int k, int end, cudaStream_t s) { return prof ? cudaEventRecord(prof->k[2 * k + end], s) : cudaSuccess; };
+  CBM_CUDA(h, rec(kKClassify, 0, st));
+  const uint32_t n_cta = (n_events + kClassifyWarps * kTileEvents - 1) / (kClassifyWarps * kTileEvents);
+  classify_kernel<<<n_cta, 32 * kClassifyWarps, 0, st>>>(p, d_off, n_events, (uint32_t)n_hits, d_nt, d_nc, d_ac, scr.d_ctrl,
+                                                         scr.d_list[kClsM], scr.d_list[kClsH], scr.d_list[kClsG]);
+  CBM_CUDA(h, rec(kKClassify, 1, st));
+  if (!serial) {
+    CBM_CUDA(h, cudaEventRecord(h->ev_fork, st));
+    for (auto& sd : h->st_side) CBM_CUDA(h, cudaStreamWaitEvent(sd, h->ev_fork, 0));
+  }
+  // G and M first: on most workloads their persistent CTAs find a short list and leave at once
+  CBM_CUDA(h, rec(kKTeamG, 0, s_g));
+  TEAM_KERNEL_G<<<h->grid[kClsG], 32 * SmemG::W, sizeof(SmemG), s_g>>>(
+      p, d_x, d_y, d_off, d_nt, d_nc, d_ac, scr.d_ctrl, scr.d_list[kClsG], scr.d_list[kClsX], scr.d_spill[0]);
+  CBM_CUDA(h, rec(kKTeamG, 1, s_g));
+  CBM_CUDA(h, rec(kKTeamM, 0, s_m));
+  TEAM_KERNEL_M<<<h->grid[kClsM], 32 * SmemM::W, 0, s_m>>>(
+      p, d_x, d_y, d_off, d_nt, d_nc, d_ac, scr.d_ctrl, scr.d_list[kClsM], scr.d_list[kClsX], nullptr);
+  CBM_CUDA(h, rec(kKTeamM, 1, s_m));
+  CBM_CUDA(h, rec(kKTeamH, 0, st));
+  TEAM_KERNEL_H<<<h->grid[kClsH], 32 * SmemH::W, 0, st>>>(
+      p, d_x, d_y, d_off, d_nt, d_nc, d_ac, scr.d_ctrl, scr.d_list[kClsH], scr.d_list[kClsX], nullptr);
+  CBM_CUDA(h, rec(kKTeamH, 1, st));
+  if (p.tiny_max_total) {
+    CBM_CUDA(h, rec(kKTile, 0, s_tile));
+    const uint32_t n_tiles = (n_events + kTileEvents - 1) / kTileEvents;
+    if (p.S <= 4)  // tables sized for 4 stations: more resident CTAs
+      tile_kernel<4><<<n_tiles, kTileEvents * p.S, 0, s_tile>>>(p, d_x, d_y, d_off, n_events, (uint32_t)n_hits, d_nt, d_nc,
+                                                                d_ac, scr.d_ctrl, scr.d_list[kClsX]);
+    else
+      tile_kernel<kMaxStations><<<n_tiles, kTileEvents * p.S, 0, s_tile>>>(p, d_x, d_y, d_off, n_events, (uint32_t)n_hits, d_nt,
+                                                                           d_nc, d_ac, scr.d_ctrl, scr.d_list[kClsX]);
+    CBM_CUDA(h, rec(kKTile, 1, s_tile));
+  } else if (prof) {
+    CBM_CUDA(h, rec(kKTile, 0, s_tile));
+    CBM_CUDA(h, rec(kKTile, 1, s_tile));
+  }
+  if (!serial)
+    for (int i = 0; i < 3; ++i) {
+      CBM_CUDA(h, cudaEventRecord(h->ev_join[i], h->st_side[i]));
+      CBM_CUDA(h, cudaStreamWaitEvent(st, h->ev_join[i], 0));
+    }
+  CBM_CUDA(h, rec(kKTeamX, 0, st));
+  TEAM_KERNEL_X<<<h->grid[kClsX], 32 * SmemG::W, sizeof(SmemG), st>>>(
+      p, d_x, d_y, d_off, d_nt, d_nc, d_ac, scr.d_ctrl, scr.d_list[kClsX], scr.d_list[kClsX], scr.d_spill[1]);
+  CBM_CUDA(h, rec(kKTeamX, 1, st));
+  if (prof) prof->valid = true;
   CBM_CUDA(h, cudaGetLastError());
-  return 4;
+  return CBM_TRIGGER_N_KERNELS;
 }
 
 // The list of selected events: ascending ids of the events with accept != 0, and their number.
@@ -344,11 +372,11 @@ void fill_stats(cbm_trigger_stats_t& st, const Ctrl& c, uint32_t n_events, uint6
   st.struct_size = sizeof(st);
   st.n_events = n_events;
   st.n_hits = n_hits;
+  st.n_class[0] = c.n_tiny;
   st.n_class[1] = c.count[kClsM]; st.n_class[2] = c.count[kClsH]; st.n_class[3] = c.count[kClsG];
+  st.n_redone = c.count[kClsX];
   st.n_invalid = c.n_invalid;
   st.first_invalid = c.first_invalid_inv ? ~c.first_invalid_inv : 0xFFFFFFFFu;
-  // escalated events were first handled by the tile kernel, then redone by team_M
-  st.n_class[0] = n_events - (c.count[kClsM] - c.n_escalated) - c.count[kClsH] - c.count[kClsG] - c.n_invalid;
   st.n_launches = n_launches;
 }
 
@@ -381,7 +409,7 @@ int occupancy_grid(cbm_trigger* h, K kernel, int threads, size_t smem, int* grid
 // ================================================================================================ C ABI
 extern "C" {
 
-const char* cbm_trigger_version(void) { return "cbm-trigger 0.1 sm_100a"; }
+const char* cbm_trigger_version(void) { return "cbm-trigger 0.2 sm_100a"; }
 
 const char* cbm_trigger_last_error(const cbm_trigger_t* h) { return h ? h->err.c_str() : g_create_err.c_str(); }
 
@@ -420,9 +448,10 @@ int cbm_trigger_create(const cbm_trigger_config_t* cfg, cbm_trigger_t** out) {
   static_assert(sizeof(SmemM) <= 48 * 1024 && sizeof(SmemH) <= 48 * 1024, "static shared memory limit");
   CREATE_CUDA(cudaFuncSetAttribute(tile_kernel<4>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
   CREATE_CUDA(cudaFuncSetAttribute(tile_kernel<kMaxStations>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
-  CREATE_TRY(occupancy_grid(h, TEAM_KERNEL_M, 32 * kWM, 0, &h->grid[kClsM]));
-  CREATE_TRY(occupancy_grid(h, TEAM_KERNEL_H, 32 * kWH, 0, &h->grid[kClsH]));
-  CREATE_TRY(occupancy_grid(h, TEAM_KERNEL_G, 32 * kWG, sizeof(SmemG), &h->grid[kClsG]));
+  CREATE_TRY(occupancy_grid(h, TEAM_KERNEL_M, 32 * SmemM::W, 0, &h->grid[kClsM]));
+  CREATE_TRY(occupancy_grid(h, TEAM_KERNEL_H, 32 * SmemH::W, 0, &h->grid[kClsH]));
+  CREATE_TRY(occupancy_grid(h, TEAM_KERNEL_G, 32 * SmemG::W, sizeof(SmemG), &h->grid[kClsG]));
+  CREATE_TRY(occupancy_grid(h, TEAM_KERNEL_X, 32 * SmemG::W, sizeof(SmemG), &h->grid[kClsX]));
   CREATE_CUDA(cudaStreamCreateWithFlags(&h->st_h2d, cudaStreamNonBlocking));
   CREATE_CUDA(cudaStreamCreateWithFlags(&h->st_run, cudaStreamNonBlocking));
   CREATE_CUDA(cudaStreamCreateWithFlags(&h->st_d2h, cudaStreamNonBlocking));
@@ -743,7 +772,7 @@ int cbm_trigger_device_status(cbm_trigger_t* h, void* stream, cbm_trigger_stats_
   CBM_CUDA(h, cudaSetDevice(h->cfg.device));
   CBM_CUDA(h, cudaMemcpyAsync(h->h_dev_ctrl, h->dev_scr.d_ctrl, sizeof(Ctrl), cudaMemcpyDeviceToHost, (cudaStream_t)stream));
   CBM_CUDA(h, cudaStreamSynchronize((cudaStream_t)stream));
-  fill_stats(*stats, *h->h_dev_ctrl, h->dev_n_events, h->dev_n_hits, h->dev_n_events ? 4 : 0);
+  fill_stats(*stats, *h->h_dev_ctrl, h->dev_n_events, h->dev_n_hits, h->dev_n_events ? CBM_TRIGGER_N_KERNELS : 0);
   if ((h->cfg.flags & CBM_FLAG_PROFILE) && h->dev_prof_head)
     fill_prof(*stats, h->dev_prof[(h->dev_prof_head - 1) % CBM_TRIGGER_PROFILE_RING], false);
   if (stats->n_invalid)

@@ -54,14 +54,14 @@ def oracle_list_mt(geo, x, y, off, ids, n_threads=None):
 
 
 def gpu_select(layer_z, x, y, off, win_in=(1, 100), win_link=(2, 100), min_candidates=2, max_hits_per_layer=4096,
-               flags=0, tiny_max_layer_hits=0, slope_range_milli=0, check=True):
+               flags=0, tiny_max_layer_hits=0, check=True):
     """One batch through cbm_trigger_create / upload_events / run / fetch_results."""
     L = len(layer_z)
     n_events = (off.size - 1) // L
     n_hits = int(off[-1])
     trig = K.Trigger(layer_z, max(n_events, 1), max(n_hits, 1), win_in=win_in, win_link=win_link,
                      min_candidates=min_candidates, max_hits_per_layer=max_hits_per_layer, n_slots=1, flags=flags,
-                     tiny_max_layer_hits=tiny_max_layer_hits, slope_range_milli=slope_range_milli)
+                     tiny_max_layer_hits=tiny_max_layer_hits)
     try:
         x = np.ascontiguousarray(x, dtype=np.int32)
         y = np.ascontiguousarray(y, dtype=np.int32)
