@@ -42,6 +42,7 @@ def parse_args():
     ap.add_argument("--events", type=int, default=0, help="events per batch (0 = the config's size)")
     ap.add_argument("--e2e-steps", type=int, default=0, help="steps of the end-to-end leg (0 = min(steps, 10))")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--serial", action="store_true", help="CBM_FLAG_SERIAL: the kernels of a step one after the other")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-packed", action="store_true", help="skip the end-to-end leg with the packed wire format XY20")
     return ap.parse_args()
@@ -272,7 +273,7 @@ def run_ours(args, cfg, cid):
 
     trig = K.Trigger(cfg.layer_z, E, n_hits, win_in=cfg.win_in, win_link=cfg.win_link,
                      min_candidates=cfg.min_candidates, max_hits_per_layer=cfg.max_hits_per_layer, n_slots=0,
-                     device=local_rank, flags=K.CBM_FLAG_PROFILE)
+                     device=local_rank, flags=K.CBM_FLAG_PROFILE | (K.CBM_FLAG_SERIAL if args.serial else 0))
     stream = torch.cuda.Stream(device=dev)
     sampler = ClockSampler(local_rank)
     sampler.start()  # nvidia-smi needs ~0.1 s to deliver its first sample: started before the warm-up

@@ -18,6 +18,7 @@
 #include "classify.cuh"
 #include "tile.cuh"
 #include "team.cuh"
+#include "chain.cuh"
 #include "select.cuh"
 #include "wire.cuh"
 #include "msd.cuh"
@@ -26,15 +27,18 @@ namespace {
 
 using namespace cbm;
 
-// team classes (team.cuh): warps per team, fullest layer admitted, kept middle hits, band width (log2 cell
-// columns), kept hits per band, overflow band, middle hits with triplets per station, resident CTAs per SM
-using SmemM = TeamSmem<1, 128, 64, 3, 8, 32, 32>;
-using SmemH = TeamSmem<4, 448, 192, 2, 16, 64, 48>;
-using SmemG = TeamSmem<16, 4096, 4096, 0, 32, 4096, 256>;
+// team classes (team.cuh): warps per team, fullest layer admitted, kept middle hits, coarse table (log2
+// columns, log2 rows), middle hits with triplets per station
+using SmemM = TeamSmem<1, 128, 64, 4, 4, 32>;
+using SmemH = TeamSmem<4, 448, 192, 5, 5, 48>;
+using SmemG = TeamSmem<16, 4096, 4104, 5, 5, 256>;
 constexpr int kCapM = SmemM::CAP, kCapH = SmemH::CAP, kCapG = SmemG::CAP;
-constexpr int kMinBM = 24, kMinBH = 10, kMinBG = 1;
+constexpr int kMinBM = 24, kMinBH = 9, kMinBG = 1;
 #define TEAM_KERNEL_M team_kernel<SmemM, kClsM, kMinBM, false, true>
 #define TEAM_KERNEL_H team_kernel<SmemH, kClsH, kMinBH, false, true>
+// class H, round-1 design (chain.cuh): 4 warps, 448 hits per layer, 32 x 32 coarse cells, 64 list entries, 8 CTAs/SM
+using SmemHC = ChainSmem<4, 448, 32, 64>;
+#define CHAIN_KERNEL_H chain_kernel<4, 448, 32, 64, kClsH, 8, true>
 #define TEAM_KERNEL_G team_kernel<SmemG, kClsG, kMinBG, true, false>
 #define TEAM_KERNEL_X team_kernel<SmemG, kClsX, kMinBG, true, false>
 // kernels of one run, in the order of cbm_trigger_stats_t::kernel_ms
@@ -46,7 +50,8 @@ enum SlotState { kEmpty = 0, kUploaded = 1, kRunning = 2 };
 struct Scratch {
   Ctrl* d_ctrl = nullptr;
   uint32_t* d_list[kNumLists] = {nullptr, nullptr, nullptr, nullptr};  // M, H, G, X
-  uint32_t* d_spill[2] = {nullptr, nullptr};  // class G, list X; per CTA: middle-hit lists beyond shared memory
+  uint32_t* d_spill[3] = {nullptr, nullptr, nullptr};  // class G, list X, class H (chain kernel); per CTA: middle-hit
+                                                       // lists beyond shared memory
   uint32_t* d_selcnt = nullptr;  // accepted events per block of kSelEvents events (select.cuh)
   uint32_t* d_hitbase = nullptr; // first hit of every selected event in the gathered batch (select.cuh)
 };
@@ -89,6 +94,8 @@ struct cbm_trigger {
   Params p;
   int n_sm = 0;
   int grid[kNumLists] = {0, 0, 0, 0};
+  int grid_hc = 0;          // chain_kernel (class H)
+  bool h_chain = true;      // class H runs chain_kernel (default) or team_kernel (CBM_TRIGGER_H_IMPL=team)
   Slot slot[CBM_TRIGGER_MAX_SLOTS];
   Scratch dev_scr;          // scratch of cbm_trigger_run_device
   Ctrl* h_dev_ctrl = nullptr;
@@ -212,6 +219,7 @@ int alloc_scratch(cbm_trigger* h, Scratch& s) {
   for (int c = 0; c < kNumLists; ++c) CBM_CUDA(h, cudaMalloc(&s.d_list[c], (size_t)h->cfg.max_events * sizeof(uint32_t)));
   CBM_CUDA(h, cudaMalloc(&s.d_spill[0], (size_t)h->grid[kClsG] * 6 * kCapG * sizeof(uint32_t)));
   CBM_CUDA(h, cudaMalloc(&s.d_spill[1], (size_t)h->grid[kClsX] * 6 * kCapG * sizeof(uint32_t)));
+  CBM_CUDA(h, cudaMalloc(&s.d_spill[2], (size_t)h->grid_hc * 6 * kCapH * sizeof(uint32_t)));
   return CBM_OK;
 }
 void free_scratch(Scratch& s) {
@@ -219,8 +227,7 @@ void free_scratch(Scratch& s) {
   cudaFree(s.d_selcnt);
   cudaFree(s.d_hitbase);
   for (int c = 0; c < kNumLists; ++c) cudaFree(s.d_list[c]);
-  cudaFree(s.d_spill[0]);
-  cudaFree(s.d_spill[1]);
+  for (auto& sp : s.d_spill) cudaFree(sp);
   s = Scratch();
 }
 int make_prof(cbm_trigger* h, ProfEvents& pe) {
@@ -322,8 +329,12 @@ int launch_selection(cbm_trigger* h, const Scratch& scr, const int32_t* d_x, con
       p, d_x, d_y, d_off, d_nt, d_nc, d_ac, scr.d_ctrl, scr.d_list[kClsM], scr.d_list[kClsX], nullptr);
   CBM_CUDA(h, rec(kKTeamM, 1, s_m));
   CBM_CUDA(h, rec(kKTeamH, 0, st));
-  TEAM_KERNEL_H<<<h->grid[kClsH], 32 * SmemH::W, 0, st>>>(
-      p, d_x, d_y, d_off, d_nt, d_nc, d_ac, scr.d_ctrl, scr.d_list[kClsH], scr.d_list[kClsX], nullptr);
+  if (h->h_chain)
+    CHAIN_KERNEL_H<<<h->grid_hc, 32 * SmemH::W, 0, st>>>(p, d_x, d_y, d_off, d_nt, d_nc, d_ac, scr.d_ctrl, scr.d_list[kClsH],
+                                                        scr.d_spill[2]);
+  else
+    TEAM_KERNEL_H<<<h->grid[kClsH], 32 * SmemH::W, 0, st>>>(
+        p, d_x, d_y, d_off, d_nt, d_nc, d_ac, scr.d_ctrl, scr.d_list[kClsH], scr.d_list[kClsX], nullptr);
   CBM_CUDA(h, rec(kKTeamH, 1, st));
   if (p.tiny_max_total) {
     CBM_CUDA(h, rec(kKTile, 0, s_tile));
@@ -445,11 +456,16 @@ int cbm_trigger_create(const cbm_trigger_config_t* cfg, cbm_trigger_t** out) {
   CREATE_CUDA(cudaGetDeviceProperties(&prop, cfg->device));
   if (prop.major < 10) { fail(h, CBM_ERR_CUDA, "device is sm_%d%d; this library holds sm_100a code only", prop.major, prop.minor); return bail(CBM_ERR_CUDA); }
   h->n_sm = prop.multiProcessorCount;
-  static_assert(sizeof(SmemM) <= 48 * 1024 && sizeof(SmemH) <= 48 * 1024, "static shared memory limit");
+  static_assert(sizeof(SmemM) <= 48 * 1024 && sizeof(SmemH) <= 48 * 1024 && sizeof(SmemHC) <= 48 * 1024, "static shared memory limit");
   CREATE_CUDA(cudaFuncSetAttribute(tile_kernel<4>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
   CREATE_CUDA(cudaFuncSetAttribute(tile_kernel<kMaxStations>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
   CREATE_TRY(occupancy_grid(h, TEAM_KERNEL_M, 32 * SmemM::W, 0, &h->grid[kClsM]));
   CREATE_TRY(occupancy_grid(h, TEAM_KERNEL_H, 32 * SmemH::W, 0, &h->grid[kClsH]));
+  CREATE_TRY(occupancy_grid(h, CHAIN_KERNEL_H, 32 * SmemH::W, 0, &h->grid_hc));
+  {
+    const char* impl = getenv("CBM_TRIGGER_H_IMPL");  // tuning: "team" runs class H on team_kernel
+    h->h_chain = !(impl && strcmp(impl, "team") == 0);
+  }
   CREATE_TRY(occupancy_grid(h, TEAM_KERNEL_G, 32 * SmemG::W, sizeof(SmemG), &h->grid[kClsG]));
   CREATE_TRY(occupancy_grid(h, TEAM_KERNEL_X, 32 * SmemG::W, sizeof(SmemG), &h->grid[kClsX]));
   CREATE_CUDA(cudaStreamCreateWithFlags(&h->st_h2d, cudaStreamNonBlocking));

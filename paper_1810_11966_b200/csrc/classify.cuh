@@ -70,20 +70,33 @@ __global__ void __launch_bounds__(32 * kClassifyWarps)
   const bool tiny = tile_admit(p, lane, in, invalid, mx, tot);
   int cls = -1;
   if (in && !invalid && !tiny) cls = mx <= p.cls_max[kClsM] ? kClsM : (mx <= p.cls_max[kClsH] ? kClsH : kClsG);
-  uint32_t* const lists[kNumTeamClasses] = {list_M, list_H, list_G};
+  // List positions: counts per warp and class -> one atomicAdd per class and CTA -> every lane's slot.  The order
+  // inside a list is irrelevant: results are indexed by event, one writer per address.
+  __shared__ uint32_t wcnt[kClassifyWarps][kNumTeamClasses + 1];  // [warp][class], [3] = tiny
+  __shared__ uint32_t cbase[kNumTeamClasses];
+  uint32_t bal[kNumTeamClasses];
 #pragma unroll
-  for (int c = 0; c < kNumTeamClasses; ++c) {  // order inside a list is irrelevant: results are indexed by event
-    const uint32_t m = __ballot_sync(FULL, cls == c);
-    if (m) {
-      const int leader = __ffs(m) - 1;
-      uint32_t base = 0;
-      if ((int)lane == leader) base = atomicAdd(&ctrl->count[c], __popc(m));
-      base = __shfl_sync(FULL, base, leader);
-      if (cls == c) lists[c][base + __popc(m & lanemask_lt())] = e;
-    }
-  }
+  for (int c = 0; c < kNumTeamClasses; ++c) bal[c] = __ballot_sync(FULL, cls == c);
   const uint32_t tm = __ballot_sync(FULL, tiny);
-  if (tm && lane == 0) atomicAdd(&ctrl->n_tiny, __popc(tm));
+  if (lane == 0) {
+#pragma unroll
+    for (int c = 0; c < kNumTeamClasses; ++c) wcnt[warp][c] = __popc(bal[c]);
+    wcnt[warp][kNumTeamClasses] = __popc(tm);
+  }
+  __syncthreads();
+  if (tid <= kNumTeamClasses) {
+    uint32_t tot = 0;
+    for (int w = 0; w < kClassifyWarps; ++w) tot += wcnt[w][tid];
+    if (tid < kNumTeamClasses) cbase[tid] = tot ? atomicAdd(&ctrl->count[tid], tot) : 0u;
+    else if (tot) atomicAdd(&ctrl->n_tiny, tot);
+  }
+  __syncthreads();
+  if (cls >= 0) {
+    const uint32_t mine = cls == kClsM ? bal[kClsM] : (cls == kClsH ? bal[kClsH] : bal[kClsG]);
+    uint32_t pos = cbase[cls] + __popc(mine & lanemask_lt());
+    for (uint32_t w = 0; w < warp; ++w) pos += wcnt[w][cls];
+    (cls == kClsM ? list_M : (cls == kClsH ? list_H : list_G))[pos] = e;
+  }
   if (invalid) {  // rejected on the device: outputs 0, reported by fetch_results / device_status
     for (uint32_t k = 0; k < S; ++k) n_triplets[(size_t)e * S + k] = 0;
     n_candidates[e] = 0;
