@@ -30,7 +30,12 @@
  * A handle is not thread-safe; different slots may be driven from one thread as a software pipeline.
  *
  * Arithmetic range: the device evaluates |x_h*z_B - x_g*z_A| <= floor(a*z_A*z_B/b) in int64, which is exact
- * for any int32 x, y and 0 < z <= 2^23 (|D| < 2^56).  (The CPU oracle's b*|D| form needs |x|,|y| <= 2^23.)
+ * for any int32 x, y and 0 < z <= 2^23 (|D| < 2^56); no coordinate-range check is needed or made.
+ *
+ * Where input errors are found (reading B1): upload_events checks O(1) facts on the host (capacity,
+ * off[0] == 0, off[n_events*L] == n_hits); the O(E*L) structural checks (offsets non-decreasing and <= n_hits,
+ * no layer above max_hits_per_layer) run on the device inside `run` (classify_kernel reads off[] anyway) and are
+ * reported by fetch_results / device_status as CBM_ERR_RANGE.
  */
 #ifndef CBM_TRIGGER_H
 #define CBM_TRIGGER_H
@@ -110,7 +115,11 @@ void cbm_trigger_destroy(cbm_trigger_t* h);
 /* Zero-copy staging: HOST pointers into the slot's pinned buffers (owned by the handle; capacity max_hits int32
  * for x and y, max_events*L+1 uint32 for off).  A producer (DAQ / generator) writes a batch there and then calls
  * upload_events with these same pointers, which skips the staging memcpy.  (data are delivered
- * into host memory, then transferred.) */
+ * into host memory, then transferred.)
+ * Contract: between upload_events(slot) and the next fetch_results(slot) the slot's host buffers are the source of
+ * an H2D copy that may still be in flight: the producer must not write them in that interval (upload_events
+ * itself waits for the slot's previous copy before it touches them).  The handle's compute-side streams and
+ * fork/join events are shared by all slots and by run_device: runs of one handle are serialised on the device. */
 int cbm_trigger_host_buffers(cbm_trigger_t* h, uint32_t slot, int32_t** x, int32_t** y, uint32_t** off);
 
 /* a1+a2: enqueue the H2D copy of one batch into `slot` on the slot's copy stream.
@@ -167,8 +176,10 @@ int cbm_trigger_select_device(cbm_trigger_t* h, uint32_t n_events, const uint8_t
  * *d_n_selected: the count is read on the device, no host synchronisation).  Out, same layout restricted to the
  * selected events in list order: d_out_off[n_selected*L + 1] (starts at 0; room for n_events*L + 1 uint32),
  * d_out_x / d_out_y (room for all n_hits int32 in the worst case), *d_out_n_hits (uint64) = hits gathered.
- * No atomics: the output is unique.  Asynchronous; uses the handle's scratch (stream-ordered calls only). */
-int cbm_trigger_gather_device(cbm_trigger_t* h, uint32_t n_events, const int32_t* d_x, const int32_t* d_y,
+ * No atomics: the output is unique.  Asynchronous; uses the handle's scratch (stream-ordered calls only).
+ * The list is not trusted: at most n_events entries are read, and an id >= n_events or an event whose extent
+ * off[e*L] .. off[e*L+L] is not inside [0, n_hits] is gathered as an empty event. */
+int cbm_trigger_gather_device(cbm_trigger_t* h, uint32_t n_events, uint64_t n_hits, const int32_t* d_x, const int32_t* d_y,
                               const uint32_t* d_off, const uint32_t* d_event_ids, const uint32_t* d_n_selected,
                               int32_t* d_out_x, int32_t* d_out_y, uint32_t* d_out_off, unsigned long long* d_out_n_hits,
                               void* stream);
@@ -181,8 +192,8 @@ int cbm_trigger_gather_device(cbm_trigger_t* h, uint32_t n_events, const int32_t
  *   3. d_accept[e] = d_n_passing[e] >= min_triplets (2)
  * evaluated exactly: with Svz = sum v_i z_i, Szz = sum z_i^2, Svv = sum v_i^2 over the three hits,
  *   den * (Szz*Svv - Svz^2) <= num * 10^6 * ndf * Szz      (thr = num/den cm^2; 10-um units; 128-bit integers),
- * which needs |x|, |y| <= 2^23.  d_n_passing[n_events] uint32 = min(2^32-1, passing triplets); d_accept uint8.
- * An event with malformed offsets selects nothing.  Asynchronous. */
+ * exact for any int32 x, y.  d_n_passing[n_events] uint32 = min(2^32-1, passing triplets); d_accept uint8.
+ * An event with malformed offsets has d_n_passing = 0 and d_accept = 0 (also with min_triplets = 0).  Asynchronous. */
 typedef struct {
   uint32_t struct_size;            /* = sizeof(cbm_trigger_msd_params_t) */
   uint32_t station;                /* the trigger station, 0..S-1; 0xFFFFFFFF = the last one */

@@ -27,7 +27,7 @@
  *   outputs: n_triplets[e*S+s] = min(2^32-1, |T_s|), n_candidates[e] = min(2^32-1, candidates),
  *            accept[e] = n_candidates[e] >= min_candidates
  *
- * All arithmetic is int64 / uint64; there is no floating point, no sorting, no
+ * All arithmetic is integer (int64 / uint64, the window products in 128 bits); there is no floating point, no sorting, no
  * blocking.  The only shortcut is the (h0,h1) short-circuit before the h2 loop.
  *
  * Pins (tests/test_oracle_pins.py): brute force without any short-circuit and with
@@ -55,12 +55,14 @@ typedef struct {
 
 static int64_t iabs64(int64_t v) { return v < 0 ? -v : v; }
 
-/* compat(): |x_h/z_A - x_g/z_B| <= a/b and the same in y, cross-multiplied (z > 0). */
+/* compat(): |x_h/z_A - x_g/z_B| <= a/b and the same in y, cross-multiplied (z > 0).
+ * The products b*|D| are formed in 128 bits so that the definition holds for every int32 coordinate
+ * (|D| < 2^56, b <= 2^12; reading B2), not only for |x|, |y| <= 2^23. */
 static int compat(int64_t xh, int64_t yh, int64_t zA, int64_t xg, int64_t yg, int64_t zB,
                   int64_t a, int64_t b) {
-  int64_t rhs = a * zA * zB;
-  if (b * iabs64(xh * zB - xg * zA) > rhs) return 0;
-  if (b * iabs64(yh * zB - yg * zA) > rhs) return 0;
+  __int128 rhs = (__int128)a * zA * zB;
+  if ((__int128)b * iabs64(xh * zB - xg * zA) > rhs) return 0;
+  if ((__int128)b * iabs64(yh * zB - yg * zA) > rhs) return 0;
   return 1;
 }
 

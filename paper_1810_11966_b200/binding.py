@@ -137,7 +137,7 @@ def load_library():
         lib.cbm_trigger_select_device.restype = i32
         lib.cbm_trigger_select_device.argtypes = [vp, u32, vp, vp, vp, vp]
         lib.cbm_trigger_gather_device.restype = i32
-        lib.cbm_trigger_gather_device.argtypes = [vp, u32, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
+        lib.cbm_trigger_gather_device.argtypes = [vp, u32, u64, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
         lib.cbm_trigger_msd_device.restype = i32
         lib.cbm_trigger_msd_device.argtypes = [vp, ctypes.POINTER(MsdParams), u32, u64, vp, vp, vp, vp, vp, vp]
         lib.cbm_trigger_get_stats.restype = i32
@@ -256,10 +256,10 @@ def cbm_trigger_select_device(handle, n_events, d_accept, d_event_ids, d_n_selec
     _check(load_library().cbm_trigger_select_device(handle, n_events, d_accept, d_event_ids, d_n_selected, stream), handle)
 
 
-def cbm_trigger_gather_device(handle, n_events, d_x, d_y, d_off, d_ids, d_n_sel, d_out_x, d_out_y, d_out_off, d_out_n_hits,
-                              stream=0):
+def cbm_trigger_gather_device(handle, n_events, n_hits, d_x, d_y, d_off, d_ids, d_n_sel, d_out_x, d_out_y, d_out_off,
+                              d_out_n_hits, stream=0):
     """d_* are raw device addresses (ints); stream is a cudaStream_t as int."""
-    _check(load_library().cbm_trigger_gather_device(handle, n_events, d_x, d_y, d_off, d_ids, d_n_sel, d_out_x, d_out_y,
+    _check(load_library().cbm_trigger_gather_device(handle, n_events, n_hits, d_x, d_y, d_off, d_ids, d_n_sel, d_out_x, d_out_y,
                                                     d_out_off, d_out_n_hits, stream), handle)
 
 
@@ -383,11 +383,11 @@ class Trigger:
         cbm_trigger_run_device(self.handle, n_events, n_hits, d_x.data_ptr(), d_y.data_ptr(), d_off.data_ptr(),
                                d_nt.data_ptr(), d_nc.data_ptr(), d_ac.data_ptr(), st)
 
-    def gather_device(self, n_events, d_x, d_y, d_off, d_ids, d_n, d_ox, d_oy, d_ooff, d_on, stream=None):
+    def gather_device(self, n_events, n_hits, d_x, d_y, d_off, d_ids, d_n, d_ox, d_oy, d_ooff, d_on, stream=None):
         """The selected events' hits as a compact batch (torch CUDA tensors)."""
         import torch
         st = torch.cuda.current_stream().cuda_stream if stream is None else stream
-        cbm_trigger_gather_device(self.handle, n_events, d_x.data_ptr(), d_y.data_ptr(), d_off.data_ptr(), d_ids.data_ptr(),
+        cbm_trigger_gather_device(self.handle, n_events, n_hits, d_x.data_ptr(), d_y.data_ptr(), d_off.data_ptr(), d_ids.data_ptr(),
                                   d_n.data_ptr(), d_ox.data_ptr(), d_oy.data_ptr(), d_ooff.data_ptr(), d_on.data_ptr(), st)
 
     def msd_device(self, params, n_events, n_hits, d_x, d_y, d_off, d_np, d_ac, stream=None):

@@ -6,6 +6,7 @@
 // without a CUDA device cbm_trigger_create fails with CBM_ERR_CUDA.
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
@@ -697,12 +698,13 @@ int cbm_trigger_select_device(cbm_trigger_t* h, uint32_t n_events, const uint8_t
   return nl < 0 ? nl : CBM_OK;
 }
 
-int cbm_trigger_gather_device(cbm_trigger_t* h, uint32_t n_events, const int32_t* d_x, const int32_t* d_y,
+int cbm_trigger_gather_device(cbm_trigger_t* h, uint32_t n_events, uint64_t n_hits, const int32_t* d_x, const int32_t* d_y,
                               const uint32_t* d_off, const uint32_t* d_event_ids, const uint32_t* d_n_selected,
                               int32_t* d_out_x, int32_t* d_out_y, uint32_t* d_out_off, unsigned long long* d_out_n_hits,
                               void* stream) {
   if (!h) return CBM_ERR_INVALID_ARG;
   if (n_events > h->cfg.max_events) return fail(h, CBM_ERR_CAPACITY, "n_events %u > max_events %u", n_events, h->cfg.max_events);
+  if (n_hits >= (1ull << 32)) return fail(h, CBM_ERR_CAPACITY, "n_hits must be < 2^32");
   if (!d_n_selected || !d_out_off || !d_out_n_hits || (n_events && (!d_off || !d_event_ids || !d_x || !d_y || !d_out_x || !d_out_y)))
     return fail(h, CBM_ERR_INVALID_ARG, "device pointers must not be NULL");
   static_assert(kGatherEvents == kSelEvents, "the per-block scratch is shared with the selection list");
@@ -710,11 +712,11 @@ int cbm_trigger_gather_device(cbm_trigger_t* h, uint32_t n_events, const int32_t
   cudaStream_t st = (cudaStream_t)stream;
   const uint32_t nb = n_events / kGatherEvents + 1;
   const Scratch& scr = h->dev_scr;
-  gather_size_kernel<<<nb, kSelThreads, 0, st>>>(d_off, h->p.L, d_event_ids, d_n_selected, scr.d_selcnt);
-  gather_base_kernel<<<nb, kSelThreads, 0, st>>>(d_off, h->p.L, d_event_ids, d_n_selected, scr.d_selcnt, scr.d_hitbase,
+  gather_size_kernel<<<nb, kSelThreads, 0, st>>>(d_off, h->p.L, n_events, (uint32_t)n_hits, d_event_ids, d_n_selected, scr.d_selcnt);
+  gather_base_kernel<<<nb, kSelThreads, 0, st>>>(d_off, h->p.L, n_events, (uint32_t)n_hits, d_event_ids, d_n_selected, scr.d_selcnt, scr.d_hitbase,
                                                  d_out_off, d_out_n_hits);
   if (n_events)
-    gather_copy_kernel<<<h->n_sm * 8, kSelThreads, 0, st>>>(d_x, d_y, d_off, h->p.L, d_event_ids, d_n_selected,
+    gather_copy_kernel<<<h->n_sm * 8, kSelThreads, 0, st>>>(d_x, d_y, d_off, h->p.L, n_events, (uint32_t)n_hits, d_event_ids, d_n_selected,
                                                             scr.d_hitbase, d_out_x, d_out_y, d_out_off);
   CBM_CUDA(h, cudaGetLastError());
   return CBM_OK;

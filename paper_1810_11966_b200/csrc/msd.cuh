@@ -6,7 +6,8 @@
 // Exact form of the cut (the paper's floating-point precision is unstated; B8): with Svz = sum v_i z_i,
 // Szz = sum z_i^2, Svv = sum v_i^2 over the three hits, the sum of squared residuals of the fitted line is
 // Svv - Svz^2/Szz, and  MSD/ndf <= num/den cm^2  <=>  den*(Szz*Svv - Svz^2) <= num*10^6*ndf*Szz  in 10-um units:
-// 128-bit integers (|v|, z <= 2^23: left < 2^108, right < 2^92).
+// 128-bit integers; exact for any int32 coordinates and 0 < z <= 2^23 (Svz < 2^56 in int64, Svv < 2^64 in uint64,
+// Szz*Svv < 2^112, left side < 2^124, right side < 2^92).
 //
 // One warp per event; lane <-> (h0,h1) pair.  A passing triplet has every residual |r_i| <= delta = sqrt(thr*ndf),
 // hence |v1*z0 - v0*z1| = |r1*z0 - r0*z1| <= delta*(z0+z1): an exact 64-bit necessary condition on the pair that
@@ -29,9 +30,9 @@ constexpr int kMsdWarps = 4;
 __device__ __forceinline__ bool msd_ok(int64_t v0, int64_t v1, int64_t v2, int64_t z0, int64_t z1, int64_t z2, int64_t szz,
                                        uint32_t num, uint32_t den, uint32_t ndf) {
   const int64_t svz = v0 * z0 + v1 * z1 + v2 * z2;
-  const int64_t svv = v0 * v0 + v1 * v1 + v2 * v2;
+  const uint64_t svv = (uint64_t)(v0 * v0) + (uint64_t)(v1 * v1) + (uint64_t)(v2 * v2);  // < 3 * 2^62
   const uint64_t asvz = (uint64_t)(svz < 0 ? -svz : svz);
-  const unsigned __int128 ssr_szz = (unsigned __int128)(uint64_t)szz * (uint64_t)svv - (unsigned __int128)asvz * asvz;  // >= 0
+  const unsigned __int128 ssr_szz = (unsigned __int128)(uint64_t)szz * svv - (unsigned __int128)asvz * asvz;  // >= 0
   const unsigned __int128 lhs = ssr_szz * den;
   const unsigned __int128 rhs = (unsigned __int128)((uint64_t)num * 1000000ull * ndf) * (uint64_t)szz;
   return lhs <= rhs;
@@ -46,7 +47,8 @@ __global__ void __launch_bounds__(32 * kMsdWarps)
   const uint32_t* o = off + (size_t)e * p.L + p.first_layer;
   const uint32_t o0 = __ldg(o), o1 = __ldg(o + 1), o2 = __ldg(o + 2), o3 = __ldg(o + 3);
   unsigned long long cnt = 0;
-  if ((o0 <= o1) & (o1 <= o2) & (o2 <= o3) & (o3 <= n_hits)) {  // a malformed event selects nothing
+  const bool well_formed = (o0 <= o1) & (o1 <= o2) & (o2 <= o3) & (o3 <= n_hits);
+  if (well_formed) {  // a malformed event selects nothing and is never accepted
     const uint32_t n1 = o2 - o1;
     const unsigned long long n_pairs = (unsigned long long)(o1 - o0) * n1;
     const int64_t z0 = p.z0, z1 = p.z1, z2 = p.z2;
@@ -72,7 +74,7 @@ __global__ void __launch_bounds__(32 * kMsdWarps)
   if (lane == 0) {
     const uint32_t c = cnt > 0xFFFFFFFFull ? 0xFFFFFFFFu : (uint32_t)cnt;
     n_passing[e] = c;
-    accept[e] = c >= p.min_triplets ? 1 : 0;
+    accept[e] = (well_formed && c >= p.min_triplets) ? 1 : 0;
   }
 }
 

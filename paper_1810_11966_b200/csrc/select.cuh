@@ -93,30 +93,35 @@ __global__ void __launch_bounds__(kSelThreads)
 constexpr int kGatherPerThread = 16;
 constexpr int kGatherEvents = kSelThreads * kGatherPerThread;
 
-__device__ __forceinline__ uint32_t gather_event_size(const uint32_t* __restrict__ off, uint32_t L, uint32_t e) {
-  return __ldg(off + (size_t)e * L + L) - __ldg(off + (size_t)e * L);
+// Hits of selected event e; 0 for an id beyond the batch or an event whose extent is not inside [0, n_hits]
+// (caller-supplied ids and offsets are not trusted: such an event is gathered as empty).
+__device__ __forceinline__ uint32_t gather_event_size(const uint32_t* __restrict__ off, uint32_t L, uint32_t e, uint32_t n_events,
+                                                      uint32_t n_hits) {
+  if (e >= n_events) return 0u;
+  const uint32_t src = __ldg(off + (size_t)e * L), end = __ldg(off + (size_t)e * L + L);
+  return (src <= end && end <= n_hits) ? end - src : 0u;
 }
 
 __global__ void __launch_bounds__(kSelThreads)
-    gather_size_kernel(const uint32_t* __restrict__ off, uint32_t L, const uint32_t* __restrict__ ids,
-                       const uint32_t* __restrict__ n_selected, uint32_t* __restrict__ block_sum) {
+    gather_size_kernel(const uint32_t* __restrict__ off, uint32_t L, uint32_t n_events, uint32_t n_hits,
+                       const uint32_t* __restrict__ ids, const uint32_t* __restrict__ n_selected, uint32_t* __restrict__ block_sum) {
   __shared__ uint32_t warp_sums[kSelThreads / 32];
-  const uint32_t n = *n_selected;
+  const uint32_t n = min(*n_selected, n_events);
   const uint32_t first = (blockIdx.x * kSelThreads + threadIdx.x) * kGatherPerThread;
   uint32_t sum = 0;
-  for (uint32_t i = first; i < min(first + kGatherPerThread, n); ++i) sum += gather_event_size(off, L, __ldg(ids + i));
+  for (uint32_t i = first; i < min(first + kGatherPerThread, n); ++i) sum += gather_event_size(off, L, __ldg(ids + i), n_events, n_hits);
   uint32_t total;
   sel_block_exclusive_scan(sum, warp_sums, &total);
   if (threadIdx.x == 0) block_sum[blockIdx.x] = total;
 }
 
 __global__ void __launch_bounds__(kSelThreads)
-    gather_base_kernel(const uint32_t* __restrict__ off, uint32_t L, const uint32_t* __restrict__ ids,
-                       const uint32_t* __restrict__ n_selected, const uint32_t* __restrict__ block_sum,
+    gather_base_kernel(const uint32_t* __restrict__ off, uint32_t L, uint32_t n_events, uint32_t n_hits,
+                       const uint32_t* __restrict__ ids, const uint32_t* __restrict__ n_selected, const uint32_t* __restrict__ block_sum,
                        uint32_t* __restrict__ hit_base, uint32_t* __restrict__ out_off, unsigned long long* __restrict__ out_n_hits) {
   __shared__ uint32_t warp_sums[kSelThreads / 32];
   __shared__ uint32_t base_sh;
-  const uint32_t n = *n_selected;
+  const uint32_t n = min(*n_selected, n_events);
   uint32_t part = 0;
   for (uint32_t b = threadIdx.x; b < blockIdx.x; b += kSelThreads) part += block_sum[b];
   uint32_t before;
@@ -127,7 +132,7 @@ __global__ void __launch_bounds__(kSelThreads)
   uint32_t sz[kGatherPerThread], sum = 0;
 #pragma unroll
   for (int k = 0; k < kGatherPerThread; ++k) {
-    sz[k] = first + k < n ? gather_event_size(off, L, __ldg(ids + first + k)) : 0u;
+    sz[k] = first + k < n ? gather_event_size(off, L, __ldg(ids + first + k), n_events, n_hits) : 0u;
     sum += sz[k];
   }
   uint32_t total;
@@ -148,15 +153,17 @@ __global__ void __launch_bounds__(kSelThreads)
 // one CTA per selected event (grid-stride)
 __global__ void __launch_bounds__(kSelThreads)
     gather_copy_kernel(const int32_t* __restrict__ x, const int32_t* __restrict__ y, const uint32_t* __restrict__ off,
-                       uint32_t L, const uint32_t* __restrict__ ids, const uint32_t* __restrict__ n_selected,
-                       const uint32_t* __restrict__ hit_base, int32_t* __restrict__ out_x, int32_t* __restrict__ out_y,
-                       uint32_t* __restrict__ out_off) {
-  const uint32_t n = *n_selected;
+                       uint32_t L, uint32_t n_events, uint32_t n_hits, const uint32_t* __restrict__ ids,
+                       const uint32_t* __restrict__ n_selected, const uint32_t* __restrict__ hit_base, int32_t* __restrict__ out_x,
+                       int32_t* __restrict__ out_y, uint32_t* __restrict__ out_off) {
+  const uint32_t n = min(*n_selected, n_events);
   for (uint32_t i = blockIdx.x; i < n; i += gridDim.x) {
     const uint32_t e = __ldg(ids + i), dst = hit_base[i];
-    const uint32_t src = __ldg(off + (size_t)e * L), end = __ldg(off + (size_t)e * L + L);
-    for (uint32_t l = threadIdx.x; l < L; l += kSelThreads) out_off[(size_t)i * L + l] = dst + (__ldg(off + (size_t)e * L + l) - src);
-    for (uint32_t k = threadIdx.x; k < end - src; k += kSelThreads) {
+    const uint32_t size = gather_event_size(off, L, e, n_events, n_hits);  // 0: not a well-formed event of the batch
+    const uint32_t src = size ? __ldg(off + (size_t)e * L) : 0u;
+    for (uint32_t l = threadIdx.x; l < L; l += kSelThreads)
+      out_off[(size_t)i * L + l] = dst + (size ? min(__ldg(off + (size_t)e * L + l) - src, size) : 0u);
+    for (uint32_t k = threadIdx.x; k < size; k += kSelThreads) {
       out_x[dst + k] = __ldg(x + src + k);
       out_y[dst + k] = __ldg(y + src + k);
     }

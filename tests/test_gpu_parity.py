@@ -105,6 +105,27 @@ def test_random_geometries_and_windows(seed, flags):
         assert_same(got, want, f"S={S} win_in={win_in} win_link={win_link}")
 
 
+@pytest.mark.parametrize("flags", FLAG_SETS)
+def test_full_int32_coordinate_range(flags):
+    # include/cbm_trigger.h: exact for any int32 x, y and 0 < z <= 2^23.  Hand-computed expectations:
+    # tests/test_oracle_pins.py::full_range_cases
+    from tests.test_oracle_pins import full_range_cases
+    z, win, ev, exp = full_range_cases()
+    x, y, off = W.batch_from_layers(z, ev)
+    got = gpu_select(z, x, y, off, win_in=win, win_link=win, flags=flags)
+    assert got[0][:, 0].tolist() == exp and got[1].tolist() == exp
+    assert_same(got, oracle_of(z, x, y, off, win_in=win, win_link=win), "full int32 range")
+    # the same hits inside fuller layers (class M / H kernels): 200 background hits per layer far away in y
+    rng = np.random.default_rng(5)
+    big = []
+    for e in ev:
+        big.append([lay + [(int(rng.integers(-2**31, 2**31)), int(rng.integers(2_000_000_000, 2**31))) for _ in range(n)]
+                    for lay, n in zip(e, (200, 40, 130))])
+    x, y, off = W.batch_from_layers(z, big)
+    got = gpu_select(z, x, y, off, win_in=win, win_link=win, flags=flags)
+    assert_same(got, oracle_of(z, x, y, off, win_in=win, win_link=win), "full int32 range, full layers")
+
+
 def test_saturation_closed_forms():
     # narrow cone: every combination passes => |T_s| = n0*n1*n2, candidates = prod |T_s|
     rng = np.random.default_rng(7)

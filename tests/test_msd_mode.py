@@ -196,3 +196,28 @@ def test_msd_mode_near_the_threshold_and_edges():
         hx, hy, ho = one_event([[0], [0], [d]], [[0], [0], [0]])
         got_n, got_a = _gpu_msd(Z3, hx, hy, ho, 1, min_triplets=1)
         assert got_n.tolist() == [w] and got_a.tolist() == [w]
+
+
+@pytest.mark.gpu
+def test_msd_malformed_event_is_never_accepted():
+    """include/cbm_trigger.h: an event with malformed offsets has n_passing = 0 and accept = 0, also with
+    min_triplets = 0 (which accepts every well-formed event)."""
+    import torch
+    cfg = W.CONFIGS[0]
+    n = 40
+    b = W.generate(cfg, n_events=n)
+    L = cfg.n_layers
+    off = b.off.copy()
+    off[7 * L + (L - 2)] = off[7 * L + (L - 1)] + 5   # trigger station of event 7: offsets not monotone
+    par = K.make_msd_params(min_triplets=0)
+    with K.Trigger(cfg.layer_z, n, b.n_hits, n_slots=0) as trig:
+        dx = torch.from_numpy(np.concatenate([b.x, np.zeros(8, np.int32)])).cuda()
+        dy = torch.from_numpy(np.concatenate([b.y, np.zeros(8, np.int32)])).cuda()
+        do = torch.from_numpy(off.view(np.int32)).cuda()
+        dnp = torch.full((n,), 9, dtype=torch.int32, device="cuda")
+        dac = torch.full((n,), 9, dtype=torch.uint8, device="cuda")
+        trig.msd_device(par, n, b.n_hits, dx, dy, do, dnp, dac)
+        torch.cuda.synchronize()
+        ac = dac.cpu().numpy()
+        assert ac[7] == 0 and int(dnp[7].item()) == 0
+        assert ac[np.arange(n) != 7].all()

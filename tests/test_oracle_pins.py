@@ -56,6 +56,41 @@ def test_boundary_equality_in_station_x():
     assert run_events(z, ev)[0].tolist() == [[1]]
 
 
+def full_range_cases():
+    """Hand-computed cases at the edge of the int32 coordinate range (reading B2): z0 = 8 000 000,
+    z1 = 8 200 000, z2 = 8 388 608 = 2^23, window 4095/4096.  b*|D| reaches 2^67 here, beyond int64.
+    Returns (layer_z, win_in, events, expected triplets per event)."""
+    z = [8_000_000, 8_200_000, 8_388_608]
+    X = 2**31 - 1
+    ev, exp = [], []
+    # far apart: slopes +268.4 and -261.9 differ by 530 >> 0.99976: no triplet.  D = X*(z0+z1) = 3.48e16,
+    # b*D = 1.43e20 = 7*2^64 + 1.36e19: an int64 product would come out NEGATIVE and pass the window.
+    ev.append([[(X, 0)], [(-X, 0)], [(X, 0)]]); exp.append(0)
+    # h0 and h2 on the line of slope +250, h1 at slope -207.6: no triplet.  Here 4096*|D| of the pairs (h0,h1) and
+    # (h1,h2) is 1.2297e20 and 1.2894e20: both wrap to a NEGATIVE int64 (D mod 2^52 >= 2^51), so a 64-bit evaluation
+    # of b*|D| <= a*z_A*z_B accepts both pairs and counts one triplet.  (Checked with Python integers.)
+    ev.append([[(2_000_000_000, 0)], [(-1_702_700_000, 0)], [(2_097_152_000, 0)]]); exp.append(0)
+    # the same line: slopes 250 exactly in all three layers (x = 250*z): one triplet
+    ev.append([[(2_000_000_000, 5)], [(2_050_000_000, 5)], [(2_097_152_000, 5)]]); exp.append(1)
+    # boundary: h0 = (0,0); h1 at slope a/b exactly: x1 = 4095*z1/4096 = 8 197 998.046875 -> not an integer, so
+    # x1 = 8 197 998 passes (below) and 8 197 999 fails (b*x1*z0 = 4096*8197999*z0 > 4095*z0*z1 <=> 4096*8197999 >
+    # 4095*8200000 = 33 579 000 000: 33 579 003 904 > 33 579 000 000 yes).  h2 = (0,0) is within the window of h0,
+    # and of h1 iff h1 is within the window of the origin direction (|x1/z1| <= a/b): the same condition.
+    ev.append([[(0, 0)], [(8_197_998, 0)], [(0, 0)]]); exp.append(1)
+    ev.append([[(0, 0)], [(8_197_999, 0)], [(0, 0)]]); exp.append(0)
+    # large offsets with a small difference: x0 = -2 000 000 000 (slope -250), x1 = -250*z1 + d, d = 8 197 998 passes
+    ev.append([[(-2_000_000_000, 0)], [(-2_050_000_000 + 8_197_998, 0)], [(-2_097_152_000, 0)]]); exp.append(1)
+    ev.append([[(-2_000_000_000, 0)], [(-2_050_000_000 + 8_197_999, 0)], [(-2_097_152_000, 0)]]); exp.append(0)
+    return z, (4095, 4096), ev, exp
+
+
+def test_compat_over_the_full_int32_range():
+    z, win, ev, exp = full_range_cases()
+    nt, nc, ac = run_events(z, ev, win_in=win, win_link=win)
+    assert nt[:, 0].tolist() == exp
+    assert nc.tolist() == exp  # one station: candidates = triplets
+
+
 def test_boundary_equality_in_station_y_and_nonzero_slopes():
     # same in y, on top of a common slope 0.2: y = 0.2*z + delta keeps differences unchanged
     z, ev = one_station_event((5, 12000), (5, 14000 + 700), (5, 16000))

@@ -164,7 +164,7 @@ def test_gather_device_matches_oracle(cid, n, minc):
         on = torch.zeros(1, dtype=torch.int64, device="cuda")
         trig.run_device(n, b.n_hits, dx, dy, do, dnt, dnc, dac)
         trig.select_device(n, dac, dids, dn)
-        trig.gather_device(n, dx, dy, do, dids, dn, ox, oy, oo, on)
+        trig.gather_device(n, b.n_hits, dx, dy, do, dids, dn, ox, oy, oo, on)
         torch.cuda.synchronize()
         ns, nh = int(dn.item()), int(on.item())
         assert ns == want_ids.size and nh == wx.size
@@ -172,3 +172,40 @@ def test_gather_device_matches_oracle(cid, n, minc):
         assert np.array_equal(oo.cpu().numpy().view(np.uint32)[:ns * L + 1], wo)
         assert np.array_equal(ox.cpu().numpy()[:nh], wx) and np.array_equal(oy.cpu().numpy()[:nh], wy)
         assert int(ox[nh].item()) == 77  # nothing written past the end
+
+
+@pytest.mark.gpu
+def test_gather_device_does_not_trust_the_list():
+    """ids beyond the batch, a count beyond n_events and events with a malformed extent are gathered as empty events;
+    nothing is read or written out of bounds (include/cbm_trigger.h)."""
+    import torch
+    cfg = W.CONFIGS[0]
+    n = 64
+    b = W.generate(cfg, n_events=n)
+    L = cfg.n_layers
+    off = b.off.copy()
+    off[5 * L + 3] = off[5 * L + L] + 7          # event 5: an inner offset beyond its end (extent itself still fine)
+    off[9 * L] = off[9 * L + L] + 1 if off[9 * L + L] + 1 < 2**32 else 0   # event 9: begins after it ends
+    ids = np.array([3, 9, 1000, 5, 2**32 - 1, 7], dtype=np.uint32)
+    with K.Trigger(cfg.layer_z, n, b.n_hits, n_slots=0) as trig:
+        dx, dy = torch.from_numpy(np.concatenate([b.x, np.zeros(8, np.int32)])).cuda(), torch.from_numpy(np.concatenate([b.y, np.zeros(8, np.int32)])).cuda()
+        do = torch.from_numpy(off.view(np.int32)).cuda()
+        dids = torch.from_numpy(np.concatenate([ids, np.zeros(n - ids.size, np.uint32)]).view(np.int32)).cuda()
+        dn = torch.tensor([1_000_000], dtype=torch.int32, device="cuda")   # a count far beyond n_events
+        ox = torch.full((b.n_hits + 1,), 77, dtype=torch.int32, device="cuda")
+        oy = torch.full((b.n_hits + 1,), 77, dtype=torch.int32, device="cuda")
+        oo = torch.full((n * L + 1,), -1, dtype=torch.int32, device="cuda")
+        on = torch.zeros(1, dtype=torch.int64, device="cuda")
+        trig.gather_device(n, b.n_hits, dx, dy, do, dids, dn, ox, oy, oo, on)
+        torch.cuda.synchronize()
+        o = oo.cpu().numpy().view(np.uint32)
+        size = lambda e: int(b.off[e * L + L] - b.off[e * L])
+        # entries: 3 ok, 9 malformed (empty), 1000 out of range (empty), 5 ok extent, 2^32-1 (empty), 7 ok, then zeros = event 0
+        want_sizes = [size(3), 0, 0, size(5), 0, size(7)] + [size(0)] * (n - ids.size)
+        got_sizes = [int(o[(i + 1) * L] - o[i * L]) for i in range(n)]
+        assert got_sizes == want_sizes
+        assert int(on.item()) == sum(want_sizes) and int(o[n * L]) == sum(want_sizes)
+        assert (np.diff(o[:n * L + 1].astype(np.int64)) >= 0).all()           # offsets stay monotone
+        x3 = ox.cpu().numpy()[:size(3)]
+        assert np.array_equal(x3, b.x[b.off[3 * L]:b.off[3 * L + L]])
+        assert int(ox[sum(want_sizes)].item()) == 77                            # nothing written past the end
