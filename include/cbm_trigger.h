@@ -227,6 +227,22 @@ int cbm_trigger_device_status(cbm_trigger_t* h, void* stream, cbm_trigger_stats_
  * Returns the number of calls written (>= 0) or a negative error code. */
 int cbm_trigger_device_kernel_times(cbm_trigger_t* h, void* stream, uint32_t n_last, float* kernel_ms);
 
+/* Measurement utility (the integer-pipe denominators of the roofline are measured on the box,
+ * not taken from a data sheet): runs four micro-benchmarks on the handle's device (8 independent dependency
+ * chains per thread, 8 CTAs of 256 threads per SM) and blocks until they are done.  Lane operations per second
+ * of the INT32 ALU pipe (IADD3 + LOP3) and of the FMA pipe (IMAD); exact window evaluations per second (one
+ * evaluation = the int64 test in x and in y, as the kernels compile it; PAPER.md:75-76 is the test it stands
+ * for); packed key tests per second.  out: HOST, struct_size set by the caller. */
+typedef struct {
+  uint32_t struct_size;  /* = sizeof(cbm_trigger_ubench_t) */
+  uint32_t n_sm;
+  double alu_lane_ops_per_s;
+  double imad_lane_ops_per_s;
+  double window_evals_per_s;
+  double packed_tests_per_s;
+} cbm_trigger_ubench_t;
+int cbm_trigger_ubench(cbm_trigger_t* h, cbm_trigger_ubench_t* out);
+
 /* Statistics of the last completed run of `slot` (call after fetch_results).  stats: HOST. */
 int cbm_trigger_get_stats(cbm_trigger_t* h, uint32_t slot, cbm_trigger_stats_t* stats);
 

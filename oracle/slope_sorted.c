@@ -14,7 +14,12 @@
  *     middle hits with multiplicities m_s[h1] (reading R8) instead of over
  *     one list entry per triplet.
  * It also returns N_eval, the number of algorithmic window evaluations of this
- * canonical sorted search, used for the ALU-roofline figure.
+ * canonical sorted search, used for the integer-pipe roofline:
+ * one per (h0,h1) pair inside the x-band, two per h2 inside the x-band of both hits of a
+ * pair that passed in y, two per pair of middle hits with triplets of consecutive
+ * stations.  (Reading: the canonical search links distinct middle hits,
+ * so the link term counts middle hits, not triplets.)  Pinned by hand counts in
+ * tests/test_oracle_pins.py::test_n_eval_hand_counts.
  *
  * Follows PAPER.md:73-76, 88 (section 3.2 steps 1-3) with the north_star's window and
  * linking; shares no code with the oracle or with the CUDA path.

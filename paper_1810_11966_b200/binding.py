@@ -25,6 +25,7 @@ EXPORTS = (
     "cbm_trigger_get_stats", "cbm_trigger_last_error", "cbm_trigger_version", "cbm_trigger_device_kernel_times",
     "cbm_trigger_fetch_selected", "cbm_trigger_select_device",
     "cbm_trigger_host_buffers_packed", "cbm_trigger_upload_events_packed", "cbm_trigger_msd_device", "cbm_trigger_gather_device",
+    "cbm_trigger_ubench",
 )
 PROFILE_RING = 32
 # scheduler classes (csrc/cbm_trigger.cu, csrc/params.h), restated for bookkeeping in bench.py only
@@ -69,6 +70,20 @@ class Stats(ctypes.Structure):
                 "n_invalid": self.n_invalid, "first_invalid": self.first_invalid, "n_launches": self.n_launches,
                 "kernel_ms": [float(v) for v in self.kernel_ms], "h2d_ms": float(self.h2d_ms),
                 "d2h_ms": float(self.d2h_ms)}
+
+
+class Ubench(ctypes.Structure):
+    _fields_ = [
+        ("struct_size", ctypes.c_uint32),
+        ("n_sm", ctypes.c_uint32),
+        ("alu_lane_ops_per_s", ctypes.c_double),
+        ("imad_lane_ops_per_s", ctypes.c_double),
+        ("window_evals_per_s", ctypes.c_double),
+        ("packed_tests_per_s", ctypes.c_double),
+    ]
+
+    def as_dict(self):
+        return {k: getattr(self, k) for k, _ in self._fields_ if k != "struct_size"}
 
 
 class MsdParams(ctypes.Structure):
@@ -140,6 +155,8 @@ def load_library():
         lib.cbm_trigger_gather_device.argtypes = [vp, u32, u64, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
         lib.cbm_trigger_msd_device.restype = i32
         lib.cbm_trigger_msd_device.argtypes = [vp, ctypes.POINTER(MsdParams), u32, u64, vp, vp, vp, vp, vp, vp]
+        lib.cbm_trigger_ubench.restype = i32
+        lib.cbm_trigger_ubench.argtypes = [vp, ctypes.POINTER(Ubench)]
         lib.cbm_trigger_get_stats.restype = i32
         lib.cbm_trigger_get_stats.argtypes = [vp, u32, ctypes.POINTER(Stats)]
         lib.cbm_trigger_last_error.restype = ctypes.c_char_p
@@ -261,6 +278,14 @@ def cbm_trigger_gather_device(handle, n_events, n_hits, d_x, d_y, d_off, d_ids, 
     """d_* are raw device addresses (ints); stream is a cudaStream_t as int."""
     _check(load_library().cbm_trigger_gather_device(handle, n_events, n_hits, d_x, d_y, d_off, d_ids, d_n_sel, d_out_x, d_out_y,
                                                     d_out_off, d_out_n_hits, stream), handle)
+
+
+def cbm_trigger_ubench(handle) -> dict:
+    """The integer-pipe micro-benchmarks (blocking); returns the rates as a dict."""
+    u = Ubench()
+    u.struct_size = ctypes.sizeof(Ubench)
+    _check(load_library().cbm_trigger_ubench(handle, ctypes.byref(u)), handle)
+    return u.as_dict()
 
 
 def cbm_trigger_msd_device(handle, params, n_events, n_hits, d_x, d_y, d_off, d_n_passing, d_accept, stream=0):
@@ -389,6 +414,9 @@ class Trigger:
         st = torch.cuda.current_stream().cuda_stream if stream is None else stream
         cbm_trigger_gather_device(self.handle, n_events, n_hits, d_x.data_ptr(), d_y.data_ptr(), d_off.data_ptr(), d_ids.data_ptr(),
                                   d_n.data_ptr(), d_ox.data_ptr(), d_oy.data_ptr(), d_ooff.data_ptr(), d_on.data_ptr(), st)
+
+    def ubench(self) -> dict:
+        return cbm_trigger_ubench(self.handle)
 
     def msd_device(self, params, n_events, n_hits, d_x, d_y, d_off, d_np, d_ac, stream=None):
         """The paper-literal selection on torch CUDA tensors."""

@@ -23,6 +23,7 @@
 #include "select.cuh"
 #include "wire.cuh"
 #include "msd.cuh"
+#include "ubench.cuh"
 
 namespace {
 
@@ -781,6 +782,48 @@ int cbm_trigger_run_device(cbm_trigger_t* h, uint32_t n_events, uint64_t n_hits,
   ++h->dev_prof_head;
   h->dev_n_events = n_events;
   h->dev_n_hits = n_hits;
+  return CBM_OK;
+}
+
+int cbm_trigger_ubench(cbm_trigger_t* h, cbm_trigger_ubench_t* out) {
+  if (!h) return CBM_ERR_INVALID_ARG;
+  if (!out || out->struct_size != sizeof(cbm_trigger_ubench_t)) return fail(h, CBM_ERR_INVALID_ARG, "ubench: NULL or bad struct_size");
+  CBM_CUDA(h, cudaSetDevice(h->cfg.device));
+  const int grid = h->n_sm * kUbCtasPerSm;
+  uint32_t* d_out = nullptr;
+  CBM_CUDA(h, cudaMalloc(&d_out, (size_t)grid * kUbThreads * sizeof(uint32_t)));
+  cudaEvent_t e0, e1;
+  CBM_CUDA(h, cudaEventCreate(&e0));
+  CBM_CUDA(h, cudaEventCreate(&e1));
+  const double lanes = (double)grid * kUbThreads * (double)kUbIter * 8.0;  // chain steps of one launch
+  auto timed = [&](int which, double* per_s, double per_step) -> cudaError_t {
+    float best = 1e30f;
+    for (int rep = 0; rep < 4; ++rep) {  // first repetition warms up
+      cudaEventRecord(e0, h->st_run);
+      switch (which) {
+        case 0: ub_alu_kernel<<<grid, kUbThreads, 0, h->st_run>>>(d_out, 0x9E3779B9u, 0x7F4A7C15u); break;
+        case 1: ub_imad_kernel<<<grid, kUbThreads, 0, h->st_run>>>(d_out, 1664525u, 1013904223u); break;
+        case 2: ub_window_kernel<<<grid, kUbThreads, 0, h->st_run>>>(d_out, 70000, 123456789012ll, 84000000ull); break;
+        default: ub_packed_kernel<<<grid, kUbThreads, 0, h->st_run>>>(d_out, 0x01230456u, 0xFE00FE00u); break;
+      }
+      cudaEventRecord(e1, h->st_run);
+      cudaError_t e = cudaEventSynchronize(e1);
+      if (e != cudaSuccess) return e;
+      float ms = 0;
+      cudaEventElapsedTime(&ms, e0, e1);
+      if (rep && ms < best) best = ms;
+    }
+    *per_s = lanes * per_step / (best * 1e-3);
+    return cudaGetLastError();
+  };
+  CBM_CUDA(h, timed(0, &out->alu_lane_ops_per_s, 2.0));      // IADD3 + LOP3
+  CBM_CUDA(h, timed(1, &out->imad_lane_ops_per_s, 1.0));     // IMAD
+  CBM_CUDA(h, timed(2, &out->window_evals_per_s, 1.0));      // one evaluation = x and y
+  CBM_CUDA(h, timed(3, &out->packed_tests_per_s, 1.0));
+  out->n_sm = (uint32_t)h->n_sm;
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  cudaFree(d_out);
   return CBM_OK;
 }
 

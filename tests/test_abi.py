@@ -43,7 +43,7 @@ def test_struct_layouts_match_header(lib):
     # sizeof() as the C compiler sees it: compile a probe with gcc against the header
     import subprocess
     import tempfile
-    src = '#include "cbm_trigger.h"\n#include <stdio.h>\nint main(){printf("%zu %zu\\n", sizeof(cbm_trigger_config_t), sizeof(cbm_trigger_stats_t));return 0;}\n'
+    src = '#include "cbm_trigger.h"\n#include <stdio.h>\nint main(){printf("%zu %zu %zu %zu\\n", sizeof(cbm_trigger_config_t), sizeof(cbm_trigger_stats_t), sizeof(cbm_trigger_ubench_t), sizeof(cbm_trigger_msd_params_t));return 0;}\n'
     with tempfile.TemporaryDirectory() as d:
         c = os.path.join(d, "p.c")
         open(c, "w").write(src)
@@ -52,6 +52,8 @@ def test_struct_layouts_match_header(lib):
         out = subprocess.run([exe], check=True, capture_output=True, text=True).stdout.split()
     assert int(out[0]) == ctypes.sizeof(K.Config)
     assert int(out[1]) == ctypes.sizeof(K.Stats)
+    assert int(out[2]) == ctypes.sizeof(K.Ubench)
+    assert int(out[3]) == ctypes.sizeof(K.MsdParams)
 
 
 def test_version(lib):

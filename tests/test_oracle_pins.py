@@ -346,3 +346,34 @@ def test_golden_files_match_live_oracle():
         nt, nc, ac = oracle.run(g, b.x, b.y, b.off)
         gt, gc, ga = read_golden(path, n, cfg.n_stations)
         assert (nt == gt).all() and (nc == gc).all() and (ac == ga).all(), path
+
+
+# ---------------------------------------------------------------- N_eval of the slope-sorted counter
+def test_n_eval_hand_counts():
+    """oracle.run_slope_sorted's evaluation counter (the work term of the integer-pipe roofline)
+    against hand counts.  Per middle hit h1: one y-evaluation for every h0 in its x-band; for every (h0,h1) that
+    passes in y, two evaluations for every h2 in the x-band of both; per pair of consecutive stations two
+    evaluations for every (middle hit with triplets of s-1) x (middle hit with triplets of s)."""
+    z1 = [60000, 70000, 80000]
+    g1 = oracle.geometry(z1, (1, 100), (2, 100), 2)
+
+    def n_eval(layer_z, g, events):
+        x, y, off = W.batch_from_layers(layer_z, events)
+        return int(oracle.run_slope_sorted(g, x, y, off)[3])
+
+    # (a) one exact line: 1 y-evaluation (h0,h1) + 2 for the single h2
+    assert n_eval(z1, g1, [A.planted_lines_event(z1, [(100, -50)])]) == 3
+    # (b) n0 = 2, n1 = 1, n2 = 2, all on the axis: 2 y-evaluations, both pass, 2 h2 each -> 2 + 2*2*2 = 10
+    assert n_eval(z1, g1, [[[(0, 0), (1, 1)], [(0, 0)], [(0, 0), (2, -1)]]]) == 10
+    # (c) an h0 outside the x-band of h1 (slope 0.02 vs 0) is never evaluated; one inside the x-band but outside
+    #     in y costs its y-evaluation only: layer 0 = {far in x, in x-band but far in y}, one h1, one h2 -> 1
+    assert n_eval(z1, g1, [[[(1200, 0), (0, 3000)], [(0, 0)], [(0, 0)]]]) == 1
+    # (d) two stations, two separated exact lines: per station 2 middle hits x (1 + 2) = 6 (the other line's hits are
+    #     outside every x-band); link: 2 x 2 middle hits x 2 = 8 -> 6 + 6 + 8 = 20
+    z2 = list(W.GEOMETRY_4)[:6]
+    g2 = oracle.geometry(z2, (1, 100), (2, 100), 2)
+    assert n_eval(z2, g2, [A.planted_lines_event(z2, [(-200, 10), (150, 40)])]) == 20
+    # (e) a station without a triplet stops the linking: station 0 has a line, station 1 misses layer 1 -> 3 + 0
+    ev = A.planted_lines_event(z2, [(100, 100)])
+    ev[4] = []
+    assert n_eval(z2, g2, [ev]) == 3
