@@ -14,6 +14,8 @@
 #include <cstring>
 #include <new>
 #include <string>
+#include <thread>
+#include <vector>
 
 #include "../../include/cbm_trigger.h"
 #include "classify.cuh"
@@ -114,6 +116,24 @@ struct cbm_trigger {
 namespace {
 
 thread_local std::string g_create_err;
+
+// Staging copy of caller memory into a slot's pinned buffer: large copies are split over a few host threads (one
+// thread moves about 13 GB/s, well below the H2D link it feeds).
+void staging_copy(void* dst, const void* src, size_t bytes) {
+  constexpr size_t kMinPerThread = 32u << 20;
+  size_t n_thr = std::min<size_t>(8, bytes / kMinPerThread);
+  const unsigned hw = std::thread::hardware_concurrency();
+  if (hw) n_thr = std::min<size_t>(n_thr, hw);
+  if (n_thr < 2) { memcpy(dst, src, bytes); return; }
+  std::vector<std::thread> th;
+  const size_t per = ((bytes / n_thr) + 4095) & ~(size_t)4095;
+  for (size_t i = 0; i < n_thr; ++i) {
+    const size_t a = i * per, b = std::min(bytes, a + per);
+    if (a >= b) break;
+    th.emplace_back([=] { memcpy((char*)dst + a, (const char*)src + a, b - a); });
+  }
+  for (auto& x : th) x.join();
+}
 
 int fail(cbm_trigger* h, int code, const char* fmt, ...) {
   char buf[512];
@@ -539,9 +559,9 @@ int cbm_trigger_upload_events(cbm_trigger_t* h, uint32_t slot, uint32_t n_events
   CBM_CUDA(h, cudaSetDevice(h->cfg.device));
   // the staging buffers may still be the source of the slot's previous H2D
   CBM_CUDA(h, cudaEventSynchronize(s.ev_h2d));
-  if (x != s.h_x && n_hits) memcpy(s.h_x, x, n_hits * 4);
-  if (y != s.h_y && n_hits) memcpy(s.h_y, y, n_hits * 4);
-  if (off != s.h_off) memcpy(s.h_off, off, n_off * 4);
+  if (x != s.h_x && n_hits) staging_copy(s.h_x, x, n_hits * 4);
+  if (y != s.h_y && n_hits) staging_copy(s.h_y, y, n_hits * 4);
+  if (off != s.h_off) staging_copy(s.h_off, off, n_off * 4);
   // the device arrays may still be read by the slot's previous kernels
   CBM_CUDA(h, cudaStreamWaitEvent(h->st_h2d, s.ev_run, 0));
   const bool prof = h->cfg.flags & CBM_FLAG_PROFILE;
@@ -585,8 +605,8 @@ int cbm_trigger_upload_events_packed(cbm_trigger_t* h, uint32_t slot, uint32_t n
   CBM_CUDA(h, cudaSetDevice(h->cfg.device));
   CBM_CUDA(h, cudaEventSynchronize(s.ev_h2d));  // the staging buffers may still be the source of the previous H2D
   const size_t n_bytes = (size_t)n_hits * 5, n_copy = (size_t)((n_hits + 3) / 4) * 20;  // whole 20-byte groups
-  if (xy20 != s.h_p && n_hits) memcpy(s.h_p, xy20, n_bytes);
-  if (off != s.h_off) memcpy(s.h_off, off, n_off * 4);
+  if (xy20 != s.h_p && n_hits) staging_copy(s.h_p, xy20, n_bytes);
+  if (off != s.h_off) staging_copy(s.h_off, off, n_off * 4);
   CBM_CUDA(h, cudaStreamWaitEvent(h->st_h2d, s.ev_run, 0));  // the device arrays may still be read by the previous kernels
   const bool prof = h->cfg.flags & CBM_FLAG_PROFILE;
   if (prof) CBM_CUDA(h, cudaEventRecord(s.prof.h2d[0], h->st_h2d));

@@ -98,6 +98,14 @@ CONFIGS = {
 }
 
 
+# The paper's own measurement workload ("about 15 hits per layer", about 45 per event in the
+# trigger station; Table 1: 1 000 .. 80 000 events): one station of three layers, background
+# Poisson(15) per layer, a planted pair in 1 % of the events.  Synthetic stand-in for the sample D2; used by the
+# paper-literal MSD mode only (bench.py --mode msd, tests/test_msd_mode.py).
+PAPER_TABLE1 = WorkloadConfig("paper_table1_trigger_station", 40_000, 11, tuple(station_layers_z([210])), 0, 15.0,
+                              signal_fraction=0.01)
+
+
 def build(force: bool = False) -> str:
     """Compile gen.c into libcbmgen.so (gcc, in-tree)."""
     if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):

@@ -85,3 +85,53 @@ def assert_same(got, want, what=""):
             bad = np.argwhere(g != w)
             first = tuple(bad[0])
             raise AssertionError(f"{what}: {name} differs at {len(bad)} places; first {first}: gpu {g[first]} oracle {w[first]}")
+
+
+def oracle_msd_mt(par, x, y, off, n_threads=None, chunk=20000):
+    """oracle.run_msd over all events on all host cores."""
+    n_events = (off.size - 1) // (3 * par.n_stations)
+    npass = np.zeros(n_events, dtype=np.uint32)
+    ac = np.zeros(n_events, dtype=np.uint8)
+    n_threads = n_threads or min(32, os.cpu_count() or 1)
+    ranges = [(a, min(a + chunk, n_events)) for a in range(0, n_events, chunk)]
+
+    def work(r):
+        a, b = r
+        npass[a:b], ac[a:b] = oracle.run_msd(par, x, y, off, a, b)
+
+    with ThreadPoolExecutor(n_threads) as ex:
+        list(ex.map(work, ranges))
+    return npass, ac
+
+
+def device_run(cfg, b, flags=0):
+    """One batch through cbm_trigger_run_device on torch-owned device arrays (bench.py's launch configuration).
+    Returns (n_triplets[E][S], n_candidates[E], accept[E], stats dict)."""
+    import torch
+    E, S = b.n_events, cfg.n_stations
+    dev = torch.device("cuda:0")
+    pad = (-b.n_hits) % 4 + 4
+    dx = torch.zeros(b.n_hits + pad, dtype=torch.int32, device=dev)
+    dy = torch.zeros(b.n_hits + pad, dtype=torch.int32, device=dev)
+    dx[:b.n_hits] = torch.from_numpy(b.x).to(dev)
+    dy[:b.n_hits] = torch.from_numpy(b.y).to(dev)
+    doff = torch.from_numpy(b.off.view(np.int32)).to(dev)
+    dnt = torch.full((E * S,), -1, dtype=torch.int32, device=dev)
+    dnc = torch.full((E,), -1, dtype=torch.int32, device=dev)
+    dac = torch.full((E,), 255, dtype=torch.uint8, device=dev)
+    with K.Trigger(cfg.layer_z, E, b.n_hits, win_in=cfg.win_in, win_link=cfg.win_link, min_candidates=cfg.min_candidates,
+                   max_hits_per_layer=cfg.max_hits_per_layer, n_slots=0, flags=flags) as trig:
+        trig.run_device(E, b.n_hits, dx, dy, doff, dnt, dnc, dac)
+        rc, st = trig.device_status()
+        assert rc == K.CBM_OK
+    return (dnt.cpu().numpy().view(np.uint32).reshape(-1, S), dnc.cpu().numpy().view(np.uint32), dac.cpu().numpy(), st.as_dict())
+
+
+def parity_sample(b, cfg, nc, ac, fraction, seed=99, h_cap=448):
+    """Event ids to recompute with the oracle when all of them would take too long: a seeded fraction of the batch,
+    every event with a candidate, every accepted event and every event of the heaviest class (a layer above h_cap)."""
+    E, L = b.n_events, cfg.n_layers
+    rng = np.random.default_rng(seed)
+    mx = np.diff(b.off.astype(np.int64)).reshape(E, L).max(axis=1)
+    return np.unique(np.concatenate([rng.choice(E, size=int(E * fraction), replace=False), np.flatnonzero(nc > 0),
+                                     np.flatnonzero(ac), np.flatnonzero(mx > h_cap)]))

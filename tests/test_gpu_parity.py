@@ -10,7 +10,7 @@ from paper_1810_11966_b200 import binding as K
 from paper_1810_11966_b200 import workloads as W
 from tests import adversarial as A
 from tests.golden_io import golden_cases, read_golden
-from tests.helpers import assert_same, gpu_select, oracle_list_mt, oracle_mt
+from tests.helpers import assert_same, device_run, gpu_select, oracle_list_mt, oracle_mt, parity_sample
 
 pytestmark = pytest.mark.gpu
 
@@ -342,41 +342,64 @@ def test_device_resident_entry_point():
     assert_same(got, host, "run_device vs upload/run/fetch")
 
 
-@pytest.mark.parametrize("cid,n_sample", [(3, 40000), (1, 6000)])
-def test_full_size_sampled_parity(cid, n_sample):
-    """Full batch of the config through the device-resident entry point (bench.py's launch configuration);
-    a seeded sample of events is recomputed one by one by the oracle; invariants are checked on all events."""
-    import torch
+# ------------------------------------------------------------------------------- every config at bench size
+@pytest.mark.parametrize("cid", [0, 1, 3])
+def test_full_size_every_event(cid):
+    """BASELINE.json configs 0, 1 and 3 at full size in bench.py's launch configuration (device-resident, kernels
+    side by side): EVERY event against the oracle (north_star: bit-exact for every config)."""
     cfg = W.CONFIGS[cid]
     b = W.generate(cfg)
-    E, S = cfg.n_events, cfg.n_stations
-    dev = torch.device("cuda:0")
-    pad = (-b.n_hits) % 4 + 4
-    dx = torch.zeros(b.n_hits + pad, dtype=torch.int32, device=dev)
-    dy = torch.zeros(b.n_hits + pad, dtype=torch.int32, device=dev)
-    dx[:b.n_hits] = torch.from_numpy(b.x).to(dev)
-    dy[:b.n_hits] = torch.from_numpy(b.y).to(dev)
-    doff = torch.from_numpy(b.off.view(np.int32)).to(dev)
-    dnt = torch.full((E * S,), -1, dtype=torch.int32, device=dev)
-    dnc = torch.full((E,), -1, dtype=torch.int32, device=dev)
-    dac = torch.full((E,), 255, dtype=torch.uint8, device=dev)
-    with K.Trigger(cfg.layer_z, E, b.n_hits, n_slots=0) as trig:
-        trig.run_device(E, b.n_hits, dx, dy, doff, dnt, dnc, dac)
-        rc, st = trig.device_status()
-        assert rc == K.CBM_OK
-    nt = dnt.cpu().numpy().view(np.uint32).reshape(-1, S)
-    nc = dnc.cpu().numpy().view(np.uint32)
-    ac = dac.cpu().numpy()
-    # invariants at any size: every output written; no chain without a triplet in every station; accept rule
-    assert ac.max() <= 1
-    assert not nc[(nt == 0).any(axis=1)].any()
-    assert np.array_equal(ac, (nc >= cfg.min_candidates).astype(np.uint8))
-    # planted complete pairs are (almost) always accepted; accepted background is rare (SURVEY section 8)
-    complete = (b.truth & 2) != 0
-    assert ac[complete].mean() > 0.99
-    rng = np.random.default_rng(99)
-    ids = np.unique(np.concatenate([rng.integers(0, E, size=n_sample), np.flatnonzero(nc > 0)[:5000],
-                                    np.flatnonzero(ac)[:5000]]))
+    nt, nc, ac, st = device_run(cfg, b)
     g = oracle.geometry(cfg.layer_z, cfg.win_in, cfg.win_link, cfg.min_candidates)
-    want = oracle_list_mt(g, b.x, b.y, b.off, ids)
-    assert_same((nt[ids], nc[ids], ac[ids]), want, f"{cfg.name} sample of {ids.size}")
+    assert_same((nt, nc, ac), oracle_mt(g, b.x, b.y, b.off), f"{cfg.name}, all {cfg.n_events} events")
+    assert sum(st["n_class"]) == cfg.n_events and st["n_invalid"] == 0
+    # the serial launch sequence gives the same results
+    assert_same(device_run(cfg, b, flags=K.CBM_FLAG_SERIAL), (nt, nc, ac), f"{cfg.name} serial launch")
+
+
+def test_full_size_config2():
+    """Config 2 (1,000,000 events of six stations, log-normal occupancy) at full size: a seeded 12 % of the events,
+    every event with a candidate, every accepted event and every class-G event against the oracle; invariants on all."""
+    cfg = W.CONFIGS[2]
+    b = W.generate(cfg)
+    nt, nc, ac, st = device_run(cfg, b)
+    assert ac.max() <= 1 and not nc[(nt == 0).any(axis=1)].any()
+    assert np.array_equal(ac, (nc >= cfg.min_candidates).astype(np.uint8))
+    assert st["n_class"][3] > 1000 and st["n_class"][1] > 800_000   # the scheduler's classes are all exercised
+    ids = parity_sample(b, cfg, nc, ac, 0.12)
+    assert ids.size >= 120_000
+    g = oracle.geometry(cfg.layer_z, cfg.win_in, cfg.win_link, cfg.min_candidates)
+    assert_same((nt[ids], nc[ids], ac[ids]), oracle_list_mt(g, b.x, b.y, b.off, ids), f"{cfg.name}: {ids.size} events")
+
+
+def test_config4_chunks_through_both_pipelines():
+    """Config 4 (streaming, seed 5): two 1,000,000-event chunks of the stream with first_event != 0 through the
+    two-slot upload / run / fetch pipeline in the int32 format AND in the packed wire format: both bit-identical on
+    every event, and against the oracle on a seeded 4 % plus every event with a candidate and every class-G event."""
+    cfg = W.CONFIGS[4]
+    E = cfg.chunk_events
+    chunks = [W.generate(cfg, n_events=E, first_event=k * E) for k in (3, 7)]
+    mh = max(b.n_hits for b in chunks)
+    S, L = cfg.n_stations, cfg.n_layers
+    results = {}
+    for packed in (False, True):
+        with K.Trigger(cfg.layer_z, E, mh, win_in=cfg.win_in, win_link=cfg.win_link, min_candidates=cfg.min_candidates,
+                       n_slots=2, flags=K.CBM_FLAG_PACKED_INPUT if packed else 0) as trig:
+            for s, b in enumerate(chunks):
+                if packed:
+                    hp, ho = trig.host_buffers_packed(s)
+                    hp[:5 * b.n_hits] = W.pack_xy20(b.x, b.y)
+                    ho[:b.off.size] = b.off
+                    trig.upload_events_packed(s, hp, ho, E, b.n_hits)
+                else:
+                    hx, hy, ho = trig.host_buffers(s)
+                    hx[:b.n_hits], hy[:b.n_hits], ho[:b.off.size] = b.x, b.y, b.off
+                    trig.upload_events(s, hx, hy, ho, E, b.n_hits)
+                trig.run(s)
+            results[packed] = [trig.fetch_results(s, E) for s in range(2)]
+    g = oracle.geometry(cfg.layer_z, cfg.win_in, cfg.win_link, cfg.min_candidates)
+    for s, b in enumerate(chunks):
+        nt, nc, ac = results[False][s]
+        assert_same(results[True][s], (nt, nc, ac), f"cfg4 chunk {s}: packed vs int32 pipeline")
+        ids = parity_sample(b, cfg, nc, ac, 0.04, seed=17 + s)
+        assert_same((nt[ids], nc[ids], ac[ids]), oracle_list_mt(g, b.x, b.y, b.off, ids), f"cfg4 chunk {s}: {ids.size} events")

@@ -203,6 +203,7 @@ def test_msd_malformed_event_is_never_accepted():
     """include/cbm_trigger.h: an event with malformed offsets has n_passing = 0 and accept = 0, also with
     min_triplets = 0 (which accepts every well-formed event)."""
     import torch
+    from paper_1810_11966_b200 import binding as K
     cfg = W.CONFIGS[0]
     n = 40
     b = W.generate(cfg, n_events=n)
@@ -221,3 +222,27 @@ def test_msd_malformed_event_is_never_accepted():
         ac = dac.cpu().numpy()
         assert ac[7] == 0 and int(dnp[7].item()) == 0
         assert ac[np.arange(n) != 7].all()
+
+
+@pytest.mark.gpu
+def test_msd_paper_table1_workload_full_size():
+    """The paper-literal mode at bench.py --mode msd size: 1,000,000 events of the Table-1-shaped workload
+    (one station, about 15 hits per layer), every event against oracle/msd_oracle.c."""
+    import torch
+    from paper_1810_11966_b200 import binding as K
+    from tests.helpers import oracle_msd_mt
+    cfg = W.PAPER_TABLE1
+    E = 1_000_000
+    b = W.generate(cfg, n_events=E)
+    assert 40 < b.n_hits / E < 50
+    dx = torch.from_numpy(np.concatenate([b.x, np.zeros(8, np.int32)])).cuda()
+    dy = torch.from_numpy(np.concatenate([b.y, np.zeros(8, np.int32)])).cuda()
+    do = torch.from_numpy(b.off.view(np.int32)).cuda()
+    dnp = torch.full((E,), -1, dtype=torch.int32, device="cuda")
+    dac = torch.full((E,), 9, dtype=torch.uint8, device="cuda")
+    with K.Trigger(cfg.layer_z, E, b.n_hits, n_slots=0) as trig:
+        trig.msd_device(K.make_msd_params(), E, b.n_hits, dx, dy, do, dnp, dac)
+        torch.cuda.synchronize()
+    want = oracle_msd_mt(oracle.msd_params(cfg.layer_z), b.x, b.y, b.off)
+    assert np.array_equal(dnp.cpu().numpy().view(np.uint32), want[0]) and np.array_equal(dac.cpu().numpy(), want[1])
+    assert 0 < int(want[1].sum()) < E // 20
