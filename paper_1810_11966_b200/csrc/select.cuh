@@ -93,13 +93,21 @@ __global__ void __launch_bounds__(kSelThreads)
 constexpr int kGatherPerThread = 16;
 constexpr int kGatherEvents = kSelThreads * kGatherPerThread;
 
-// Hits of selected event e; 0 for an id beyond the batch or an event whose extent is not inside [0, n_hits]
-// (caller-supplied ids and offsets are not trusted: such an event is gathered as empty).
+// Hits of selected event e; 0 for an id beyond the batch or an event whose offsets are not non-decreasing inside
+// [0, n_hits] (caller-supplied ids and offsets are not trusted: such an event is gathered as empty).
 __device__ __forceinline__ uint32_t gather_event_size(const uint32_t* __restrict__ off, uint32_t L, uint32_t e, uint32_t n_events,
                                                       uint32_t n_hits) {
   if (e >= n_events) return 0u;
-  const uint32_t src = __ldg(off + (size_t)e * L), end = __ldg(off + (size_t)e * L + L);
-  return (src <= end && end <= n_hits) ? end - src : 0u;
+  const uint32_t* o = off + (size_t)e * L;
+  const uint32_t src = __ldg(o);
+  uint32_t prev = src;
+  bool ok = true;
+  for (uint32_t l = 1; l <= L; ++l) {
+    const uint32_t v = __ldg(o + l);
+    ok &= prev <= v;
+    prev = v;
+  }
+  return (ok && prev <= n_hits) ? prev - src : 0u;
 }
 
 __global__ void __launch_bounds__(kSelThreads)
@@ -155,14 +163,17 @@ __global__ void __launch_bounds__(kSelThreads)
     gather_copy_kernel(const int32_t* __restrict__ x, const int32_t* __restrict__ y, const uint32_t* __restrict__ off,
                        uint32_t L, uint32_t n_events, uint32_t n_hits, const uint32_t* __restrict__ ids,
                        const uint32_t* __restrict__ n_selected, const uint32_t* __restrict__ hit_base, int32_t* __restrict__ out_x,
-                       int32_t* __restrict__ out_y, uint32_t* __restrict__ out_off) {
+                       int32_t* __restrict__ out_y, uint32_t* out_off) {
   const uint32_t n = min(*n_selected, n_events);
+  // a list that names an event more than once can gather more than the n_hits the output arrays hold: then nothing
+  // is copied (gather_base_kernel has reported the total, which tells the caller)
+  if (out_off[(size_t)n * L] > n_hits) return;
   for (uint32_t i = blockIdx.x; i < n; i += gridDim.x) {
     const uint32_t e = __ldg(ids + i), dst = hit_base[i];
-    const uint32_t size = gather_event_size(off, L, e, n_events, n_hits);  // 0: not a well-formed event of the batch
+    const uint32_t size = gather_event_size(off, L, e, n_events, n_hits);  // 0: empty, or not a well-formed event
     const uint32_t src = size ? __ldg(off + (size_t)e * L) : 0u;
     for (uint32_t l = threadIdx.x; l < L; l += kSelThreads)
-      out_off[(size_t)i * L + l] = dst + (size ? min(__ldg(off + (size_t)e * L + l) - src, size) : 0u);
+      out_off[(size_t)i * L + l] = dst + (size ? __ldg(off + (size_t)e * L + l) - src : 0u);
     for (uint32_t k = threadIdx.x; k < size; k += kSelThreads) {
       out_x[dst + k] = __ldg(x + src + k);
       out_y[dst + k] = __ldg(y + src + k);

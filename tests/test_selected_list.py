@@ -179,18 +179,19 @@ def test_gather_device_does_not_trust_the_list():
     """ids beyond the batch, a count beyond n_events and events with a malformed extent are gathered as empty events;
     nothing is read or written out of bounds (include/cbm_trigger.h)."""
     import torch
+    from paper_1810_11966_b200 import binding as K
     cfg = W.CONFIGS[0]
     n = 64
     b = W.generate(cfg, n_events=n)
     L = cfg.n_layers
     off = b.off.copy()
-    off[5 * L + 3] = off[5 * L + L] + 7          # event 5: an inner offset beyond its end (extent itself still fine)
-    off[9 * L] = off[9 * L + L] + 1 if off[9 * L + L] + 1 < 2**32 else 0   # event 9: begins after it ends
+    off[5 * L + 3] = off[5 * L + L] + 7          # event 5: an inner offset beyond its end
+    off[9 * L + 1] = off[9 * L] - 1              # event 9: offsets decrease
     ids = np.array([3, 9, 1000, 5, 2**32 - 1, 7], dtype=np.uint32)
     with K.Trigger(cfg.layer_z, n, b.n_hits, n_slots=0) as trig:
         dx, dy = torch.from_numpy(np.concatenate([b.x, np.zeros(8, np.int32)])).cuda(), torch.from_numpy(np.concatenate([b.y, np.zeros(8, np.int32)])).cuda()
         do = torch.from_numpy(off.view(np.int32)).cuda()
-        dids = torch.from_numpy(np.concatenate([ids, np.zeros(n - ids.size, np.uint32)]).view(np.int32)).cuda()
+        dids = torch.from_numpy(np.concatenate([ids, np.full(n - ids.size, 2**31 + 5, np.uint32)]).view(np.int32)).cuda()
         dn = torch.tensor([1_000_000], dtype=torch.int32, device="cuda")   # a count far beyond n_events
         ox = torch.full((b.n_hits + 1,), 77, dtype=torch.int32, device="cuda")
         oy = torch.full((b.n_hits + 1,), 77, dtype=torch.int32, device="cuda")
@@ -200,8 +201,9 @@ def test_gather_device_does_not_trust_the_list():
         torch.cuda.synchronize()
         o = oo.cpu().numpy().view(np.uint32)
         size = lambda e: int(b.off[e * L + L] - b.off[e * L])
-        # entries: 3 ok, 9 malformed (empty), 1000 out of range (empty), 5 ok extent, 2^32-1 (empty), 7 ok, then zeros = event 0
-        want_sizes = [size(3), 0, 0, size(5), 0, size(7)] + [size(0)] * (n - ids.size)
+        # entries: 3 ok, 9 malformed (empty), 1000 out of range (empty), 5 malformed (empty), 2^32-1 (empty), 7 ok, then ids
+        # beyond the batch (empty)
+        want_sizes = [size(3), 0, 0, 0, 0, size(7)] + [0] * (n - ids.size)
         got_sizes = [int(o[(i + 1) * L] - o[i * L]) for i in range(n)]
         assert got_sizes == want_sizes
         assert int(on.item()) == sum(want_sizes) and int(o[n * L]) == sum(want_sizes)
@@ -209,3 +211,15 @@ def test_gather_device_does_not_trust_the_list():
         x3 = ox.cpu().numpy()[:size(3)]
         assert np.array_equal(x3, b.x[b.off[3 * L]:b.off[3 * L + L]])
         assert int(ox[sum(want_sizes)].item()) == 77                            # nothing written past the end
+        # a list that repeats events can gather more than the batch holds: the total is reported, nothing is copied
+        sizes = np.array([size(e) if e not in (5, 9) else 0 for e in range(n)])
+        big = np.argsort(sizes)[-4:].astype(np.uint32)                          # the four largest well-formed events, 16 times each
+        total = 16 * int(sizes[big].sum())
+        assert total > b.n_hits
+        rep = torch.from_numpy(np.resize(big, n).view(np.int32)).cuda()
+        dn.fill_(n)
+        ox.fill_(77)
+        trig.gather_device(n, b.n_hits, dx, dy, do, rep, dn, ox, oy, oo, on)
+        torch.cuda.synchronize()
+        assert int(on.item()) == total
+        assert int((ox != 77).sum().item()) == 0
