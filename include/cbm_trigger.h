@@ -50,7 +50,7 @@ extern "C" {
 #define CBM_TRIGGER_MAX_LAYERS 24
 #define CBM_TRIGGER_MAX_HITS_PER_LAYER 4096
 #define CBM_TRIGGER_MAX_SLOTS 4
-#define CBM_TRIGGER_N_KERNELS 6 /* classify, tile, team_M, team_H, team_G, team_X (see cbm_trigger_stats_t) */
+#define CBM_TRIGGER_N_KERNELS 6 /* classify, tile, class M, class H, class G, list X (see cbm_trigger_stats_t) */
 #define CBM_TRIGGER_PROFILE_RING 32 /* run_device calls whose per-kernel times are kept (CBM_FLAG_PROFILE) */
 
 enum {
@@ -98,8 +98,9 @@ typedef struct {
   uint32_t n_invalid;      /* events rejected on the device (bad offsets / layer too full); their outputs are 0 */
   uint32_t first_invalid;  /* smallest such event index, 0xFFFFFFFF if none */
   uint32_t n_launches;     /* kernels launched by the last run of this slot */
-  float    kernel_ms[CBM_TRIGGER_N_KERNELS]; /* CBM_FLAG_PROFILE only: device time of classify, tile, team_M, team_H,
-                                                 team_G, team_X (CUDA events on the stream of each), else 0.  Without
+  float    kernel_ms[CBM_TRIGGER_N_KERNELS]; /* CBM_FLAG_PROFILE only: device time of classify_kernel, tile_kernel,
+                                                 team_kernel (class M), chain_kernel (class H), team_kernel (class G),
+                                                 team_kernel (list X) (CUDA events on the stream of each), else 0.  Without
                                                  CBM_FLAG_SERIAL the kernels share the GPU, so a time includes waiting */
   float    h2d_ms, d2h_ms; /* CBM_FLAG_PROFILE only */
 } cbm_trigger_stats_t;

@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(_HERE, "libcbmtrigger.so")
 
 MAX_LAYERS = 24
 N_KERNELS = 6
-KERNEL_NAMES = ("classify_kernel", "tile_kernel", "team_kernel_M", "team_kernel_H", "team_kernel_G", "team_kernel_X")
+KERNEL_NAMES = ("classify_kernel", "tile_kernel", "team_kernel_M", "chain_kernel_H", "team_kernel_G", "team_kernel_X")
 CBM_OK, CBM_ERR_INVALID_ARG, CBM_ERR_RANGE, CBM_ERR_CAPACITY, CBM_ERR_STATE, CBM_ERR_CUDA = 0, -1, -2, -3, -4, -5
 CBM_FLAG_PROFILE, CBM_FLAG_NO_TINY_PATH, CBM_FLAG_PACKED_INPUT, CBM_FLAG_SERIAL = 1, 2, 4, 8
 EXPORTS = (
