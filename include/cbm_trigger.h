@@ -187,6 +187,19 @@ int cbm_trigger_gather_device(cbm_trigger_t* h, uint32_t n_events, uint64_t n_hi
                               int32_t* d_out_x, int32_t* d_out_y, uint32_t* d_out_off, unsigned long long* d_out_n_hits,
                               void* stream);
 
+/* The input filter of the paper's implementation "i3" ("we introduced a
+ * filtering of the data ..., such that only hit data in the trigger station are transferred"), for a full-setup
+ * hit stream that lies on the DEVICE: d_xyz holds n_records records (x, y, z) of int32 (10-um units; the layout of
+ * PAPER.md:166-170), d_ev_off[n_events + 1] (uint32, non-decreasing, last = n_records) the records of every event.
+ * A record is a hit of layer l iff its z equals the handle's layer_z[l]; all other records (other detectors) are
+ * dropped.  Output: the batch layout above -- d_out_off[n_events*L + 1], and in d_out_x / d_out_y (room for n_records
+ * int32 in the worst case, 16-byte aligned and padded as for cbm_trigger_run_device) the kept hits of every event
+ * grouped by layer, in stream order inside a layer (so the output is unique) -- ready for cbm_trigger_run_device on
+ * the same stream.  An event with ev_off[e] > ev_off[e+1] or beyond n_records keeps nothing.  Asynchronous; no
+ * atomics on global memory; uses the handle's scratch (stream-ordered calls only).  n_records < 2^32. */
+int cbm_trigger_filter_device(cbm_trigger_t* h, uint32_t n_events, uint64_t n_records, const int32_t* d_xyz,
+                              const uint32_t* d_ev_off, int32_t* d_out_x, int32_t* d_out_y, uint32_t* d_out_off, void* stream);
+
 /* The paper's own selection, literally (section 3.2), on caller-owned DEVICE
  * arrays (layout and stream as cbm_trigger_run_device; geometry = the handle's layer_z):
  *   1. all triplets of the trigger station, one hit from each layer

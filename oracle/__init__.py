@@ -214,3 +214,27 @@ def gather(x, y, off, n_layers, event_ids):
             ys.extend(np.asarray(y[a:b]).tolist())
             o.append(o[-1] + (b - a))
     return np.asarray(xs, dtype=np.int32), np.asarray(ys, dtype=np.int32), np.asarray(o, dtype=np.uint32)
+
+
+def filter_layers(xyz, ev_off, layer_z):
+    """The paper's input filter (implementation "i3"): out of the full-setup hit data of every event
+    (STS and MUCH, about 5000 hits per event, records x, y, z as in PAPER.md:166-170) only the hits of the layers the
+    selection works on are kept.  A hit belongs to layer l iff its z equals layer_z[l] (z is a per-layer constant,
+    DESIGN.md reading R6); every other hit is dropped.  The kept hits of an event are grouped by layer, in the order
+    they have in the stream.  Written out as the plain loops it is.
+
+    xyz: int32 [N][3] records; ev_off: [E + 1] record offsets of the events.  Returns (x, y, off) in the batch layout of
+    include/cbm_trigger.h (off has E * L + 1 entries)."""
+    xyz = np.asarray(xyz, dtype=np.int32).reshape(-1, 3)
+    ev_off = np.asarray(ev_off).ravel().tolist()
+    lz = [int(z) for z in layer_z]
+    xs, ys, off = [], [], [0]
+    rec = xyz.tolist()
+    for e in range(len(ev_off) - 1):
+        for l in range(len(lz)):
+            for i in range(ev_off[e], ev_off[e + 1]):
+                if rec[i][2] == lz[l]:
+                    xs.append(rec[i][0])
+                    ys.append(rec[i][1])
+            off.append(len(xs))
+    return np.asarray(xs, dtype=np.int32), np.asarray(ys, dtype=np.int32), np.asarray(off, dtype=np.uint32)

@@ -25,7 +25,7 @@ EXPORTS = (
     "cbm_trigger_get_stats", "cbm_trigger_last_error", "cbm_trigger_version", "cbm_trigger_device_kernel_times",
     "cbm_trigger_fetch_selected", "cbm_trigger_select_device",
     "cbm_trigger_host_buffers_packed", "cbm_trigger_upload_events_packed", "cbm_trigger_msd_device", "cbm_trigger_gather_device",
-    "cbm_trigger_ubench",
+    "cbm_trigger_ubench", "cbm_trigger_filter_device",
 )
 PROFILE_RING = 32
 # scheduler classes (csrc/cbm_trigger.cu, csrc/params.h), restated for bookkeeping in bench.py only
@@ -155,6 +155,8 @@ def load_library():
         lib.cbm_trigger_gather_device.argtypes = [vp, u32, u64, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
         lib.cbm_trigger_msd_device.restype = i32
         lib.cbm_trigger_msd_device.argtypes = [vp, ctypes.POINTER(MsdParams), u32, u64, vp, vp, vp, vp, vp, vp]
+        lib.cbm_trigger_filter_device.restype = i32
+        lib.cbm_trigger_filter_device.argtypes = [vp, u32, u64, vp, vp, vp, vp, vp, vp]
         lib.cbm_trigger_ubench.restype = i32
         lib.cbm_trigger_ubench.argtypes = [vp, ctypes.POINTER(Ubench)]
         lib.cbm_trigger_get_stats.restype = i32
@@ -278,6 +280,12 @@ def cbm_trigger_gather_device(handle, n_events, n_hits, d_x, d_y, d_off, d_ids, 
     """d_* are raw device addresses (ints); stream is a cudaStream_t as int."""
     _check(load_library().cbm_trigger_gather_device(handle, n_events, n_hits, d_x, d_y, d_off, d_ids, d_n_sel, d_out_x, d_out_y,
                                                     d_out_off, d_out_n_hits, stream), handle)
+
+
+def cbm_trigger_filter_device(handle, n_events, n_records, d_xyz, d_ev_off, d_out_x, d_out_y, d_out_off, stream=0):
+    """d_* are raw device addresses (ints); stream is a cudaStream_t as int."""
+    _check(load_library().cbm_trigger_filter_device(handle, n_events, n_records, d_xyz, d_ev_off, d_out_x, d_out_y, d_out_off,
+                                                    stream), handle)
 
 
 def cbm_trigger_ubench(handle) -> dict:
@@ -414,6 +422,13 @@ class Trigger:
         st = torch.cuda.current_stream().cuda_stream if stream is None else stream
         cbm_trigger_gather_device(self.handle, n_events, n_hits, d_x.data_ptr(), d_y.data_ptr(), d_off.data_ptr(), d_ids.data_ptr(),
                                   d_n.data_ptr(), d_ox.data_ptr(), d_oy.data_ptr(), d_ooff.data_ptr(), d_on.data_ptr(), st)
+
+    def filter_device(self, n_events, n_records, d_xyz, d_ev_off, d_ox, d_oy, d_ooff, stream=None):
+        """The input filter on torch CUDA tensors: full-setup records -> the batch layout."""
+        import torch
+        st = torch.cuda.current_stream().cuda_stream if stream is None else stream
+        cbm_trigger_filter_device(self.handle, n_events, n_records, d_xyz.data_ptr(), d_ev_off.data_ptr(), d_ox.data_ptr(),
+                                  d_oy.data_ptr(), d_ooff.data_ptr(), st)
 
     def ubench(self) -> dict:
         return cbm_trigger_ubench(self.handle)

@@ -26,6 +26,7 @@
 #include "wire.cuh"
 #include "msd.cuh"
 #include "ubench.cuh"
+#include "filter.cuh"
 
 namespace {
 
@@ -58,6 +59,7 @@ struct Scratch {
                                                        // lists beyond shared memory
   uint32_t* d_selcnt = nullptr;  // accepted events per block of kSelEvents events (select.cuh)
   uint32_t* d_hitbase = nullptr; // first hit of every selected event in the gathered batch (select.cuh)
+  uint32_t* d_fcnt = nullptr;    // hits per (event, layer) of the input filter (filter.cuh), then per-block sums behind
 };
 
 struct ProfEvents {
@@ -238,6 +240,10 @@ int alloc_scratch(cbm_trigger* h, Scratch& s) {
   CBM_CUDA(h, cudaMalloc(&s.d_ctrl, sizeof(Ctrl)));
   CBM_CUDA(h, cudaMalloc(&s.d_selcnt, ((size_t)h->cfg.max_events / kSelEvents + 1) * sizeof(uint32_t)));
   CBM_CUDA(h, cudaMalloc(&s.d_hitbase, ((size_t)h->cfg.max_events + 1) * sizeof(uint32_t)));
+  {
+    const size_t n = (size_t)h->cfg.max_events * h->p.L;
+    CBM_CUDA(h, cudaMalloc(&s.d_fcnt, (n + n / kSelEvents + 2) * sizeof(uint32_t)));
+  }
   for (int c = 0; c < kNumLists; ++c) CBM_CUDA(h, cudaMalloc(&s.d_list[c], (size_t)h->cfg.max_events * sizeof(uint32_t)));
   CBM_CUDA(h, cudaMalloc(&s.d_spill[0], (size_t)h->grid[kClsG] * 6 * kCapG * sizeof(uint32_t)));
   CBM_CUDA(h, cudaMalloc(&s.d_spill[1], (size_t)h->grid[kClsX] * 6 * kCapG * sizeof(uint32_t)));
@@ -248,6 +254,7 @@ void free_scratch(Scratch& s) {
   cudaFree(s.d_ctrl);
   cudaFree(s.d_selcnt);
   cudaFree(s.d_hitbase);
+  cudaFree(s.d_fcnt);
   for (int c = 0; c < kNumLists; ++c) cudaFree(s.d_list[c]);
   for (auto& sp : s.d_spill) cudaFree(sp);
   s = Scratch();
@@ -739,6 +746,35 @@ int cbm_trigger_gather_device(cbm_trigger_t* h, uint32_t n_events, uint64_t n_hi
   if (n_events)
     gather_copy_kernel<<<h->n_sm * 8, kSelThreads, 0, st>>>(d_x, d_y, d_off, h->p.L, n_events, (uint32_t)n_hits, d_event_ids, d_n_selected,
                                                             scr.d_hitbase, d_out_x, d_out_y, d_out_off);
+  CBM_CUDA(h, cudaGetLastError());
+  return CBM_OK;
+}
+
+int cbm_trigger_filter_device(cbm_trigger_t* h, uint32_t n_events, uint64_t n_records, const int32_t* d_xyz,
+                              const uint32_t* d_ev_off, int32_t* d_out_x, int32_t* d_out_y, uint32_t* d_out_off, void* stream) {
+  if (!h) return CBM_ERR_INVALID_ARG;
+  if (n_events > h->cfg.max_events) return fail(h, CBM_ERR_CAPACITY, "n_events %u > max_events %u", n_events, h->cfg.max_events);
+  if (n_records >= (1ull << 32)) return fail(h, CBM_ERR_CAPACITY, "n_records must be < 2^32");
+  if (!d_out_off || (n_events && (!d_ev_off || (n_records && (!d_xyz || !d_out_x || !d_out_y)))))
+    return fail(h, CBM_ERR_INVALID_ARG, "device pointers must not be NULL");
+  CBM_CUDA(h, cudaSetDevice(h->cfg.device));
+  cudaStream_t st = (cudaStream_t)stream;
+  const uint32_t L = h->p.L;
+  if (n_events == 0) {
+    CBM_CUDA(h, cudaMemsetAsync(d_out_off, 0, sizeof(uint32_t), st));
+    return CBM_OK;
+  }
+  FilterDev fp;
+  fp.L = L;
+  for (uint32_t l = 0; l < (uint32_t)kMaxLayers; ++l) fp.z[l] = l < L ? h->p.z[l] : 0x7FFFFFFF;
+  const Scratch& scr = h->dev_scr;
+  const uint32_t n = n_events * L;  // < 2^32 (checked at create)
+  const uint32_t nb = (n + kSelEvents - 1) / kSelEvents;
+  uint32_t* const d_bsum = scr.d_fcnt + n;
+  filter_count_kernel<<<n_events, kFilterThreads, 0, st>>>(fp, d_xyz, d_ev_off, n_events, (uint32_t)n_records, scr.d_fcnt);
+  scan_sums_kernel<<<nb, kSelThreads, 0, st>>>(scr.d_fcnt, n, d_bsum);
+  scan_write_kernel<<<nb, kSelThreads, 0, st>>>(scr.d_fcnt, n, d_bsum, d_out_off);
+  filter_scatter_kernel<<<n_events, kFilterThreads, 0, st>>>(fp, d_xyz, d_ev_off, n_events, (uint32_t)n_records, d_out_off, d_out_x, d_out_y);
   CBM_CUDA(h, cudaGetLastError());
   return CBM_OK;
 }

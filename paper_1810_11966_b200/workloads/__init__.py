@@ -246,3 +246,46 @@ def pack_xy20(x, y):
         raise ValueError("coordinate outside the 20-bit range of the XY20 wire format")
     v = (x.astype(np.int64) & 0xFFFFF).astype(np.uint64) | ((y.astype(np.int64) & 0xFFFFF).astype(np.uint64) << np.uint64(20))
     return np.ascontiguousarray(v.astype("<u8").view(np.uint8).reshape(-1, 8)[:, :5]).reshape(-1)
+
+
+def full_setup_stream(batch: Batch, other_hits_per_event=400, seed=0, other_z=None):
+    """A full-setup hit stream around a generated batch (input formatting only; PAPER.md:166-170: records x, y, z;
+    PAPER.md:188: an event holds the hits of the whole setup, of which the selection uses a small fraction): every
+    event's batch hits become records (x, y, z of their layer), mixed in random order -- the relative order of the
+    hits of one layer is kept -- with `other_hits_per_event` (Poisson) records of other detector planes (z values
+    that are not layer z).  Returns (xyz int32 [N][3], ev_off uint32 [E + 1])."""
+    cfg = batch.cfg
+    L, E = cfg.n_layers, batch.n_events
+    rng = np.random.default_rng(seed)
+    lz = np.asarray(cfg.layer_z, dtype=np.int32)
+    if other_z is None:  # STS-like planes upstream of the absorbers, and planes between the stations
+        other_z = np.asarray([z for z in list(range(30_000, 101_000, 10_000)) + [int(v) + 5_000 for v in lz] if z not in set(lz.tolist())],
+                             dtype=np.int32)
+    cnt = np.diff(batch.off.astype(np.int64)).reshape(E, L)
+    n_much = cnt.sum(axis=1)
+    n_other = rng.poisson(other_hits_per_event, size=E).astype(np.int64)
+    ev_off = np.zeros(E + 1, dtype=np.int64)
+    np.cumsum(n_much + n_other, out=ev_off[1:])
+    N = int(ev_off[-1])
+    assert N < 2**32
+    xyz = np.empty((N, 3), dtype=np.int32)
+    layer_of_hit = np.repeat(np.tile(np.arange(L), E), cnt.ravel())
+    for e in range(E):
+        a, b = int(batch.off[e * L]), int(batch.off[e * L + L])
+        m, o = int(n_much[e]), int(n_other[e])
+        is_much = np.zeros(m + o, dtype=bool)
+        is_much[rng.choice(m + o, size=m, replace=False)] = True
+        # batch hits in a random layer interleaving that keeps the order inside every layer
+        order = np.argsort(rng.random(m) + 0.0, kind="stable") if m else np.zeros(0, dtype=np.int64)
+        lay = layer_of_hit[a:b]
+        seq = np.empty(m, dtype=np.int64)
+        # positions are dealt to layers at random; within a layer the hits keep their order
+        perm_lay = lay[order]
+        for l in np.unique(lay):
+            seq[np.flatnonzero(perm_lay == l)] = a + np.flatnonzero(lay == l)
+        rec = xyz[int(ev_off[e]):int(ev_off[e + 1])]
+        rec[is_much, 0], rec[is_much, 1], rec[is_much, 2] = batch.x[seq], batch.y[seq], lz[layer_of_hit[seq]]
+        rec[~is_much, 0] = rng.integers(-400_000, 400_001, size=o)
+        rec[~is_much, 1] = rng.integers(-400_000, 400_001, size=o)
+        rec[~is_much, 2] = other_z[rng.integers(0, other_z.size, size=o)]
+    return xyz, ev_off.astype(np.uint32)
