@@ -22,6 +22,7 @@
 #include "tile.cuh"
 #include "team.cuh"
 #include "chain.cuh"
+#include "station.cuh"
 #include "select.cuh"
 #include "wire.cuh"
 #include "msd.cuh"
@@ -44,6 +45,11 @@ constexpr int kMinBM = 24, kMinBH = 9, kMinBG = 1;
 // class H, round-1 design (chain.cuh): 4 warps, 448 hits per layer, 32 x 32 coarse cells, 64 list entries, 8 CTAs/SM
 using SmemHC = ChainSmem<4, 448, 32, 64>;
 #define CHAIN_KERNEL_H chain_kernel<4, 448, 32, 64, kClsH, 8, true>
+// class H, one warp per (event, station) (station.cuh): 448 hits per layer, 32 x 32 coarse cells; kStWarps warps
+// per CTA, kStMinB CTAs per SM
+using SmemHS = StationSmem<448, 5, 5>;
+constexpr int kStWarps = 4, kStMinB = 5;
+#define STATION_KERNEL_H station_kernel<SmemHS, kStWarps, kClsH, kStMinB>
 #define TEAM_KERNEL_G team_kernel<SmemG, kClsG, kMinBG, true, false>
 #define TEAM_KERNEL_X team_kernel<SmemG, kClsX, kMinBG, true, false>
 // kernels of one run, in the order of cbm_trigger_stats_t::kernel_ms
@@ -60,6 +66,9 @@ struct Scratch {
   uint32_t* d_selcnt = nullptr;  // accepted events per block of kSelEvents events (select.cuh)
   uint32_t* d_hitbase = nullptr; // first hit of every selected event in the gathered batch (select.cuh)
   uint32_t* d_fcnt = nullptr;    // hits per (event, layer) of the input filter (filter.cuh), then per-block sums behind
+  // station_kernel: per item (list position * S + station) the number of middle hits with triplets and the
+  // first kStEnt of them; per list position the number of finished stations (zero between runs)
+  uint32_t *d_st_cnt = nullptr, *d_st_ent = nullptr, *d_done = nullptr;
 };
 
 struct ProfEvents {
@@ -101,7 +110,9 @@ struct cbm_trigger {
   int n_sm = 0;
   int grid[kNumLists] = {0, 0, 0, 0};
   int grid_hc = 0;          // chain_kernel (class H)
-  bool h_chain = true;      // class H runs chain_kernel (default) or team_kernel (CBM_TRIGGER_H_IMPL=team)
+  int grid_hs = 0;          // station_kernel (class H)
+  int h_impl = 0;           // class H runs station_kernel (0, default), chain_kernel (1) or team_kernel (2):
+                            // CBM_TRIGGER_H_IMPL=station|chain|team
   Slot slot[CBM_TRIGGER_MAX_SLOTS];
   Scratch dev_scr;          // scratch of cbm_trigger_run_device
   Ctrl* h_dev_ctrl = nullptr;
@@ -248,6 +259,13 @@ int alloc_scratch(cbm_trigger* h, Scratch& s) {
   CBM_CUDA(h, cudaMalloc(&s.d_spill[0], (size_t)h->grid[kClsG] * 6 * kCapG * sizeof(uint32_t)));
   CBM_CUDA(h, cudaMalloc(&s.d_spill[1], (size_t)h->grid[kClsX] * 6 * kCapG * sizeof(uint32_t)));
   CBM_CUDA(h, cudaMalloc(&s.d_spill[2], (size_t)h->grid_hc * 6 * kCapH * sizeof(uint32_t)));
+  {
+    const size_t n_items = (size_t)h->cfg.max_events * h->p.S;
+    CBM_CUDA(h, cudaMalloc(&s.d_st_cnt, n_items * sizeof(uint32_t)));
+    CBM_CUDA(h, cudaMalloc(&s.d_st_ent, n_items * kStEnt * sizeof(uint32_t)));
+    CBM_CUDA(h, cudaMalloc(&s.d_done, (size_t)h->cfg.max_events * sizeof(uint32_t)));
+    CBM_CUDA(h, cudaMemset(s.d_done, 0, (size_t)h->cfg.max_events * sizeof(uint32_t)));
+  }
   return CBM_OK;
 }
 void free_scratch(Scratch& s) {
@@ -257,6 +275,7 @@ void free_scratch(Scratch& s) {
   cudaFree(s.d_fcnt);
   for (int c = 0; c < kNumLists; ++c) cudaFree(s.d_list[c]);
   for (auto& sp : s.d_spill) cudaFree(sp);
+  cudaFree(s.d_st_cnt); cudaFree(s.d_st_ent); cudaFree(s.d_done);
   s = Scratch();
 }
 int make_prof(cbm_trigger* h, ProfEvents& pe) {
@@ -358,7 +377,11 @@ int launch_selection(cbm_trigger* h, const Scratch& scr, const int32_t* d_x, con
       p, d_x, d_y, d_off, d_nt, d_nc, d_ac, scr.d_ctrl, scr.d_list[kClsM], scr.d_list[kClsX], nullptr);
   CBM_CUDA(h, rec(kKTeamM, 1, s_m));
   CBM_CUDA(h, rec(kKTeamH, 0, st));
-  if (h->h_chain)
+  if (h->h_impl == 0)
+    STATION_KERNEL_H<<<h->grid_hs, 32 * kStWarps, kStWarps * sizeof(SmemHS), st>>>(
+        p, d_x, d_y, d_off, d_nt, d_nc, d_ac, scr.d_ctrl, scr.d_list[kClsH], scr.d_list[kClsX], scr.d_st_cnt, scr.d_st_ent,
+        scr.d_done);
+  else if (h->h_impl == 1)
     CHAIN_KERNEL_H<<<h->grid_hc, 32 * SmemH::W, 0, st>>>(p, d_x, d_y, d_off, d_nt, d_nc, d_ac, scr.d_ctrl, scr.d_list[kClsH],
                                                         scr.d_spill[2]);
   else
@@ -449,6 +472,17 @@ int occupancy_grid(cbm_trigger* h, K kernel, int threads, size_t smem, int* grid
 // ================================================================================================ C ABI
 extern "C" {
 
+#ifdef ST_DEBUG
+void cbm_trigger_debug_dump(void) {
+  unsigned long long v[16];
+  cudaDeviceSynchronize();
+  cudaMemcpyFromSymbol(v, cbm::g_st_dbg, sizeof(v));
+  printf("ST_DEBUG rounds %llu surv %llu d2passes %llu d2items %llu joiners %llu mc0 %llu mc2 %llu slow %llu cand %llu allcand %llu over3 %llu\n", v[0], v[1], v[2], v[3], v[4], v[5], v[6], v[7], v[8], v[9], v[10]);
+  memset(v, 0, sizeof(v));
+  cudaMemcpyToSymbol(cbm::g_st_dbg, v, sizeof(v));
+}
+#endif
+
 const char* cbm_trigger_version(void) { return "cbm-trigger 0.2 sm_100a"; }
 
 const char* cbm_trigger_last_error(const cbm_trigger_t* h) { return h ? h->err.c_str() : g_create_err.c_str(); }
@@ -491,9 +525,10 @@ int cbm_trigger_create(const cbm_trigger_config_t* cfg, cbm_trigger_t** out) {
   CREATE_TRY(occupancy_grid(h, TEAM_KERNEL_M, 32 * SmemM::W, 0, &h->grid[kClsM]));
   CREATE_TRY(occupancy_grid(h, TEAM_KERNEL_H, 32 * SmemH::W, 0, &h->grid[kClsH]));
   CREATE_TRY(occupancy_grid(h, CHAIN_KERNEL_H, 32 * SmemH::W, 0, &h->grid_hc));
+  CREATE_TRY(occupancy_grid(h, STATION_KERNEL_H, 32 * kStWarps, kStWarps * sizeof(SmemHS), &h->grid_hs));
   {
-    const char* impl = getenv("CBM_TRIGGER_H_IMPL");  // tuning: "team" runs class H on team_kernel
-    h->h_chain = !(impl && strcmp(impl, "team") == 0);
+    const char* impl = getenv("CBM_TRIGGER_H_IMPL");  // tuning: the other two kernels for class H
+    h->h_impl = (impl && strcmp(impl, "team") == 0) ? 2 : (impl && strcmp(impl, "chain") == 0) ? 1 : 0;
   }
   CREATE_TRY(occupancy_grid(h, TEAM_KERNEL_G, 32 * SmemG::W, sizeof(SmemG), &h->grid[kClsG]));
   CREATE_TRY(occupancy_grid(h, TEAM_KERNEL_X, 32 * SmemG::W, sizeof(SmemG), &h->grid[kClsX]));
