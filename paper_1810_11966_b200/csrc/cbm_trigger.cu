@@ -111,8 +111,8 @@ struct cbm_trigger {
   int grid[kNumLists] = {0, 0, 0, 0};
   int grid_hc = 0;          // chain_kernel (class H)
   int grid_hs = 0;          // station_kernel (class H)
-  int h_impl = 0;           // class H runs station_kernel (0, default), chain_kernel (1) or team_kernel (2):
-                            // CBM_TRIGGER_H_IMPL=station|chain|team
+  int h_impl = 1;           // class H runs chain_kernel (1, default: the fastest measured), station_kernel (0) or
+                            // team_kernel (2): CBM_TRIGGER_H_IMPL=chain|station|team
   Slot slot[CBM_TRIGGER_MAX_SLOTS];
   Scratch dev_scr;          // scratch of cbm_trigger_run_device
   Ctrl* h_dev_ctrl = nullptr;
@@ -259,7 +259,7 @@ int alloc_scratch(cbm_trigger* h, Scratch& s) {
   CBM_CUDA(h, cudaMalloc(&s.d_spill[0], (size_t)h->grid[kClsG] * 6 * kCapG * sizeof(uint32_t)));
   CBM_CUDA(h, cudaMalloc(&s.d_spill[1], (size_t)h->grid[kClsX] * 6 * kCapG * sizeof(uint32_t)));
   CBM_CUDA(h, cudaMalloc(&s.d_spill[2], (size_t)h->grid_hc * 6 * kCapH * sizeof(uint32_t)));
-  {
+  if (h->h_impl == 0) {  // scratch of station_kernel
     const size_t n_items = (size_t)h->cfg.max_events * h->p.S;
     CBM_CUDA(h, cudaMalloc(&s.d_st_cnt, n_items * sizeof(uint32_t)));
     CBM_CUDA(h, cudaMalloc(&s.d_st_ent, n_items * kStEnt * sizeof(uint32_t)));
@@ -528,7 +528,7 @@ int cbm_trigger_create(const cbm_trigger_config_t* cfg, cbm_trigger_t** out) {
   CREATE_TRY(occupancy_grid(h, STATION_KERNEL_H, 32 * kStWarps, kStWarps * sizeof(SmemHS), &h->grid_hs));
   {
     const char* impl = getenv("CBM_TRIGGER_H_IMPL");  // tuning: the other two kernels for class H
-    h->h_impl = (impl && strcmp(impl, "team") == 0) ? 2 : (impl && strcmp(impl, "chain") == 0) ? 1 : 0;
+    h->h_impl = (impl && strcmp(impl, "team") == 0) ? 2 : (impl && strcmp(impl, "station") == 0) ? 0 : 1;
   }
   CREATE_TRY(occupancy_grid(h, TEAM_KERNEL_G, 32 * SmemG::W, sizeof(SmemG), &h->grid[kClsG]));
   CREATE_TRY(occupancy_grid(h, TEAM_KERNEL_X, 32 * SmemG::W, sizeof(SmemG), &h->grid[kClsX]));

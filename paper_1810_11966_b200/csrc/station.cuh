@@ -26,30 +26,32 @@
 // Accept/reject never uses a key, a cell or a bitmap: those only decide which pairs get the exact test, and the
 // pairs tested are a proven superset of the compatible ones.
 #pragma once
+#include <stddef.h>
 #include "ptx.cuh"
 #include "team.cuh"
 
 namespace cbm {
 
-constexpr int kStEnt = 32;  // middle hits with triplets a station list holds; an event with more goes to list X
+constexpr int kStEnt = 32;
+constexpr uint32_t kPriv = 8;  // candidates of one middle hit the fast path of phase D holds  // middle hits with triplets a station list holds; an event with more goes to list X
 
 template <int CAP_, int TXB_, int TYB_>
 struct StationSmem {
   static constexpr int CAP = CAP_, TXB = TXB_, TYB = TYB_;
   static constexpr int LCAP = CAP + 8;            // a layer as it lies in x[], from the 16-byte boundary below it
   static constexpr int NHEAD = 1 << (TXB + TYB);
-  static constexpr int KCAP = 128;                // kept middle hits per round of phases C and D
-  static constexpr int ICAP = 32 + 4 * 32;
-  static_assert(2 * LCAP + 1 < 1024 && LCAP < 512 && KCAP <= 128 && KCAP % 64 == 0, "field widths");
+  static constexpr int KCAP = 96;                 // kept middle hits per round of phases C and D
+  static_assert(2 * LCAP + 1 < 1024 && LCAP < 512 && KCAP <= 128 && KCAP % 32 == 0, "field widths");
   static_assert((long long)CAP * CAP < (1 << 18), "entry = index | triplets << 9");
   alignas(16) uint32_t node[2 * LCAP];            // layers 0 and 2: link | (kx mod 2^11) << 10 | (ky mod 2^11) << 21
   alignas(16) uint32_t head[NHEAD];               // chains of both layers: element + 1; 0 = empty
-  alignas(16) uint32_t occ[2][128];               // occupancy bitmaps, row fy = 64 bits, bit fx; after B: slots
+  alignas(16) uint32_t occ[2][128];               // occupancy bitmaps, row fy = 64 bits, bit fx; after B: the pair list
+                                                  // (middle hit | (element + 1) << 8), then the joiners of phase D4
   alignas(16) uint32_t J[128];
-  uint32_t kP[KCAP];                              // kept middle hits: packed key (kx mod 2^16 | ky mod 2^16 << 16),
-                                                  // after D1 the anchor word of the packed test
-  uint32_t items[ICAP];                           // survivor | (element + 1) << 8
-  uint16_t kI[KCAP];                              // kept middle hits: hit index in layer 1
+  alignas(8) uint32_t slot[2 * KCAP];             // [kept middle hit][layer 0, layer 2]: count << 27 | e2 << 18 | e1 << 9 | e0
+  uint32_t kP[KCAP];                              // kept middle hits: packed key (kx mod 2^16 | ky mod 2^16 << 16)
+  uint16_t kI[KCAP];                              // kept middle hits: hit index in layer 1; bit 15: slow path
+  uint16_t priv[32 * kPriv];                      // per lane: elements that passed the packed test (phase D1)
   uint32_t trash;                                 // chain head of the elements of a quad that are not hits of the layer
 };
 
@@ -182,7 +184,17 @@ __device__ unsigned long long g_st_dbg[16];
 #else
 #define ST_DBG(i, v) do { } while (0)
 #endif
-constexpr uint32_t kSlotCap = 3;  // elements a slot records: count << 27 | e2 << 18 | e1 << 9 | e0  (element + 1)
+__device__ __forceinline__ void sts_addr(uint32_t addr, uint32_t v) {
+  asm volatile("st.shared.u32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
+}
+__device__ __forceinline__ void sts_u16_addr(uint32_t addr, uint32_t v) {
+  asm volatile("{ .reg .u16 t; cvt.u16.u32 t, %1; st.shared.u16 [%0], t; }" ::"r"(addr), "r"(v) : "memory");
+}
+__device__ __forceinline__ uint32_t lds_u16_addr(uint32_t addr) {
+  uint32_t v;
+  asm volatile("{ .reg .u16 t; ld.shared.u16 t, [%1]; cvt.u32.u16 %0, t; }" : "=r"(v) : "r"(addr));
+  return v;
+}
 
 template <class SM, int WPC, int CLS, int MINB>
 __global__ void __launch_bounds__(32 * WPC, MINB)
@@ -196,12 +208,11 @@ __global__ void __launch_bounds__(32 * WPC, MINB)
   constexpr int XS = 6 - SM::TXB, YS = 6 - SM::TYB;  // fine cells per coarse cell (log2), >= 1
   constexpr uint32_t MX = (1u << SM::TXB) - 1u, MY = (1u << SM::TYB) - 1u;
   static_assert(XS >= 1 && YS >= 1, "a coarse cell spans at least two fine cells");
-  static_assert(KCAP * 2 <= 256, "the slots live in the bitmaps");
+  static_assert(32 * kPriv <= 256 && KCAP <= 256, "the pair list lives in the bitmaps");
   extern __shared__ __align__(16) unsigned char smem_dyn[];
   const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   SM& sm = reinterpret_cast<SM*>(smem_dyn)[warp];
   const uint32_t a_node = smem_u32(sm.node), a_head = smem_u32(sm.head), a_occ = smem_u32(sm.occ), a_J = smem_u32(sm.J);
-  const uint32_t a_slot = a_occ;
   const uint32_t S = p.S, L = p.L;
   const uint32_t n_items = ctrl->count[CLS] * S;
   const int fsh = p.cell_sh, R = p.key_R;
@@ -315,14 +326,12 @@ __global__ void __launch_bounds__(32 * WPC, MINB)
         if (qi + 32 < nq02) quad(qi + 32, xn, yn);
       }
       if (v2 && lane < 4) o2 = __ldg(off + (size_t)e2 * L + 3 * s2 + lane);  // used at the end of this item
-      // layer 1 in pairs from an 8-byte boundary: the first trip's loads fly during phase B
+      // layer 1, one hit per lane and trip: the first trip's loads fly during phase B
       const int32_t M1 = p.key_mul[3 * s + 1];
-      const uint32_t sp1 = b1 & 1u, h1 = b1 & ~1u;
-      const uint32_t npair1 = (sp1 + n1 + 1u) >> 1;
-      const int2* const x1p = reinterpret_cast<const int2*>(x + h1);
-      const int2* const y1p = reinterpret_cast<const int2*>(y + h1);
-      int2 xc = make_int2(0, 0), yc = xc;
-      if (lane < npair1) { xc = __ldg(x1p + lane); yc = __ldg(y1p + lane); }
+      const int32_t* const x1p = x + b1;
+      const int32_t* const y1p = y + b1;
+      int32_t xc = 0, yc = 0;
+      if (lane < n1) { xc = __ldg(x1p + lane); yc = __ldg(y1p + lane); }
       __syncwarp();
       // ---- B: J = dilate(occ0) & dilate(occ2) on the cyclic grid; lane <-> rows 2*lane, 2*lane + 1
       {
@@ -339,77 +348,78 @@ __global__ void __launch_bounds__(32 * WPC, MINB)
         }
         reinterpret_cast<uint4*>(sm.J)[lane] = make_uint4((uint32_t)j0, (uint32_t)(j0 >> 32), (uint32_t)j1, (uint32_t)(j1 >> 32));
       }
-      __syncwarp();  // from here on the bitmaps are the slots of phase D: [survivor][layer]
+      __syncwarp();  // from here on the bitmaps are the pair list of phase D
 
       const int32_t z0 = p.z[3 * s], z1 = p.z[3 * s + 1], z2 = p.z[3 * s + 2];
-      uint32_t pr0 = 0;  // pairs of layer 1 already filtered
-      while (pr0 < npair1) {
+      const uint32_t a_priv = smem_u32(sm.priv) + 2u * kPriv * lane, a_pairs = a_occ, a_kP = smem_u32(sm.kP);
+      uint32_t i1b = 0;  // hits of layer 1 already filtered
+      const int32_t* xq = x1p + lane + 32;  // this lane's hit of the next trip
+      const int32_t* yq = y1p + lane + 32;
+      while (i1b < n1) {
         // ---- C (a6): keep the middle hits whose fine cell is in J, up to KCAP per round
         uint32_t nk = 0;
-        while (pr0 < npair1) {
-          const uint32_t pi = pr0 + lane;
-          int2 xn = make_int2(0, 0), yn = xn;
-          if (pi + 32 < npair1) { xn = __ldg(x1p + pi + 32); yn = __ldg(y1p + pi + 32); }
-          const int32_t xs[2] = {xc.x, xc.y}, ys[2] = {yc.x, yc.y};
-          uint32_t km[2], P1[2];
-#pragma unroll
-          for (int k = 0; k < 2; ++k) {
-            const int kx = __mulhi(xs[k], M1), ky = __mulhi(ys[k], M1);
-            const uint32_t fx = (uint32_t)(kx >> fsh);
-            const uint32_t wi = ((uint32_t)(ky >> (fsh - 1)) & 0x7Eu) | ((fx >> 5) & 1u);
-            const uint32_t jw = lds_addr(a_J + 4u * wi);
-            const bool keep = (2 * pi + k - sp1 < n1) & ((jw >> (fx & 31u)) & 1u);  // pi >= npair1: index >= n1
-            km[k] = __ballot_sync(FULL, keep);
-            P1[k] = __byte_perm((uint32_t)kx, (uint32_t)ky, 0x5410);
+        while (i1b < n1) {
+          const uint32_t i1 = i1b + lane;
+          int32_t xn = 0, yn = 0;
+          if (i1 + 32 < n1) { xn = __ldg(xq); yn = __ldg(yq); }
+          const int kx = __mulhi(xc, M1), ky = __mulhi(yc, M1);
+          const uint32_t fx = (uint32_t)(kx >> fsh), ty = (uint32_t)(ky >> (fsh - 1));
+          const uint32_t jw = lds_addr(a_J + (((ty << 2) & 0x1F8u) | ((fx >> 3) & 4u)));
+          const bool keep = (i1 < n1) & ((jw >> (fx & 31u)) & 1u);
+          const uint32_t km = __ballot_sync(FULL, keep);
+          const uint32_t c = __popc(km);
+          if (nk + c > (uint32_t)KCAP) break;  // the round is full: this trip opens the next one
+          if (keep) {
+            const uint32_t w = nk + __popc(km & lt);
+            sm.kP[w] = __byte_perm((uint32_t)kx, (uint32_t)ky, 0x5410);
+            sm.kI[w] = (uint16_t)i1;
           }
-          const uint32_t c0 = __popc(km[0]);
-          if (nk + c0 + __popc(km[1]) > (uint32_t)KCAP) break;  // the round is full: this trip opens the next one
-          if ((km[0] >> lane) & 1u) {
-            const uint32_t w = nk + __popc(km[0] & lt);
-            sm.kP[w] = P1[0];
-            sm.kI[w] = (uint16_t)(2 * pi - sp1);
-          }
-          if ((km[1] >> lane) & 1u) {
-            const uint32_t w = nk + c0 + __popc(km[1] & lt);
-            sm.kP[w] = P1[1];
-            sm.kI[w] = (uint16_t)(2 * pi + 1u - sp1);
-          }
-          nk += c0 + __popc(km[1]);
-          pr0 += 32;
+          nk += c;
+          i1b += 32;
+          xq += 32; yq += 32;
           xc = xn; yc = yn;
         }
+        // the slots of this round: [survivor][layer] = count << 27 | e2 << 18 | e1 << 9 | e0  (hits COMPATIBLE with
+        // the middle hit, element + 1)
+        for (uint32_t i = lane; i < 2u * nk; i += 32) sm.slot[i] = 0;
         ST_DBG(0, 1); ST_DBG(1, nk);
         __syncwarp();
-        // ---- D1 / D2: heads, then the chains' further elements as items, drained in full warp passes
-        uint32_t ni = 0;
-        auto drain_items = [&](bool all) {
-          while (ni >= 32u || (all && ni)) {
-            const uint32_t take = min(ni, 32u);
-            ni -= take;
+        const int64_t T01 = p.thr_in[s][0], T02 = p.thr_in[s][1], T12 = p.thr_in[s][2];
+        const uint64_t T01x2 = p.thr2_in[s][0], T02x2 = p.thr2_in[s][1], T12x2 = p.thr2_in[s][2];
+        // ---- D3: lane <-> pair (middle hit, element that passed the packed test): exact test, slot of the middle hit
+        uint32_t np = 0;
+        auto drain_pairs = [&](bool all) {
+          while (np >= 32u || (all && np)) {
+            const uint32_t take = min(np, 32u);
+            np -= take;
             ST_DBG(2, 1); ST_DBG(3, take);
             __syncwarp();
-            uint32_t k = 0, link = 0;
             if (lane < take) {
-              const uint32_t it = sm.items[ni + lane];
-              k = it & 0xFFu;
-              const uint32_t el1 = it >> 8;  // element + 1
-              const uint32_t w = lds_addr(a_node + 4u * el1 - 4u);
-              link = w & 0x3FFu;
-              if (((sm.kP[k] - w) & nmask) == 0) {
-                const bool side = el1 > (uint32_t)LCAP;
-                const uint32_t a_sl = a_slot + 8u * k + (side ? 4u : 0u);
-                if ((lds_addr(a_sl) >> 27) <= kSlotCap) {  // at most 4 items of a middle hit per pass: no wrap
+              const uint32_t pr = lds_addr(a_pairs + 4u * (np + lane));
+              const uint32_t k = pr & 0xFFu, el1 = pr >> 8;
+              const bool side = el1 > (uint32_t)LCAP;                 // element of layer 2
+              const uint32_t j1 = el1 - (side ? (uint32_t)LCAP : 0u);  // element in its layer (from the quad base) + 1
+              const uint32_t gi = (side ? g2 : g0) + j1 - 1u;
+              const uint32_t i1 = sm.kI[k] & 0x7FFFu;
+              const int32_t x1 = __ldg(x1p + i1), y1 = __ldg(y1p + i1);
+              const int32_t xe = __ldg(x + gi), ye = __ldg(y + gi);
+              // |x_e*z1 - x1*z_e| <= T_e1
+              const int32_t ze = side ? z2 : z0;
+              const int64_t Te = side ? T12 : T01;
+              const uint64_t Te2 = side ? T12x2 : T01x2;
+              if (win_q(xe, z1, anchor_q(x1, -ze, Te), Te2) & win_q(ye, z1, anchor_q(y1, -ze, Te), Te2)) {
+                // a pass holds at most kPriv pairs of one middle hit: with the check the count stays below 2^5
+                const uint32_t a_sl = smem_u32(sm.slot) + 8u * k + (side ? 4u : 0u);
+                if ((lds_addr(a_sl) >> 27) <= 3u) {
                   const uint32_t c = atoms_add_addr(a_sl, 1u << 27) >> 27;
-                  if (c < kSlotCap) atoms_add_addr(a_sl, (el1 - (side ? (uint32_t)LCAP : 0u)) << (9u * c));
+                  if (c < 3u) atoms_add_addr(a_sl, j1 << (9u * c));
                 }
               }
             }
-            const uint32_t cm = __ballot_sync(FULL, link != 0);
-            __syncwarp();
-            if (link) sm.items[ni + __popc(cm & lt)] = k | (link << 8);
-            ni += __popc(cm);
           }
         };
+        // ---- D1: lane <-> kept middle hit: the chains of the <= 2 x 2 coarse cells its window touches; elements that
+        // pass the packed test go to the lane's private list, then all lists are packed into the pair list
         for (uint32_t kb = 0; kb < nk; kb += 32) {
           const uint32_t k = kb + lane;
           uint32_t hv[4] = {0, 0, 0, 0};
@@ -421,123 +431,118 @@ __global__ void __launch_bounds__(32 * WPC, MINB)
             // key_R <= 2^cell_sh and a coarse cell is >= 2^(cell_sh+1) wide: at most two columns and two rows (cyclic)
             const uint32_t lox = ((kx - R) >> (fsh + XS)) & MX, hix = ((kx + R) >> (fsh + XS)) & MX;
             const uint32_t loy = ((ky - R) >> (fsh + YS)) & MY, hiy = ((ky + R) >> (fsh + YS)) & MY;
-            hv[0] = sm.head[(lox << SM::TYB) | loy];
-            if (hiy != loy) hv[1] = sm.head[(lox << SM::TYB) | hiy];
+            const uint32_t a_lo = a_head + (lox << (SM::TYB + 2)), a_hi = a_head + (hix << (SM::TYB + 2));
+            hv[0] = lds_addr(a_lo + 4u * loy);
+            if (hiy != loy) hv[1] = lds_addr(a_lo + 4u * hiy);
             if (hix != lox) {
-              hv[2] = sm.head[(hix << SM::TYB) | loy];
-              if (hiy != loy) hv[3] = sm.head[(hix << SM::TYB) | hiy];
+              hv[2] = lds_addr(a_hi + 4u * loy);
+              if (hiy != loy) hv[3] = lds_addr(a_hi + 4u * hiy);
             }
           }
-          uint32_t sl[2] = {0, 0};  // this middle hit's slots (layer 0, layer 2), in registers for the heads
-          uint32_t lk[4];
+          uint32_t c = 0;        // entries of the private list (kPriv hold; more: the middle hit takes the slow path)
+          uint32_t a_pw = a_priv;
+          auto test = [&](uint32_t el1) {  // element el1 - 1: packed test, private list; returns its chain link
+            const uint32_t w = lds_addr(a_node + 4u * el1 - 4u);
+            if (((A - w) & nmask) == 0) {
+              if (c < kPriv) sts_u16_addr(a_pw, el1);
+              a_pw += 2u;
+              ++c;
+            }
+            return w & 0x3FFu;
+          };
+          uint32_t rem[4];
 #pragma unroll
-          for (int c = 0; c < 4; ++c) {
-            lk[c] = 0;
-            if (hv[c]) {
-              const uint32_t w = lds_addr(a_node + 4u * hv[c] - 4u);
-              lk[c] = w & 0x3FFu;
-              if (((A - w) & nmask) == 0) {
-                const bool side = hv[c] > (uint32_t)LCAP;
-                const uint32_t j1 = hv[c] - (side ? (uint32_t)LCAP : 0u);  // element in its layer + 1
-                uint32_t& r = side ? sl[1] : sl[0];
-                if ((r >> 27) < kSlotCap) r += j1 << (9u * (r >> 27));  // a fourth one is counted, not recorded
-                r += 1u << 27;
-              }
+          for (int q = 0; q < 4; ++q) {  // the first two elements of every chain, straight-line
+            rem[q] = 0;
+            if (hv[q]) {
+              const uint32_t l1 = test(hv[q]);
+              if (l1) rem[q] = test(l1);
             }
           }
-          if (k < nk) {
-            sm.kP[k] = A;
-            *reinterpret_cast<uint2*>(&sm.occ[0][0] + 2 * k) = make_uint2(sl[0], sl[1]);
-          }
+          while (__any_sync(FULL, (rem[0] | rem[1] | rem[2] | rem[3]) != 0)) {  // chains of three and more: rare
 #pragma unroll
-          for (int c = 0; c < 4; ++c) {
-            const uint32_t m = __ballot_sync(FULL, lk[c] != 0);
-            if (lk[c]) sm.items[ni + __popc(m & lt)] = k | (lk[c] << 8);
-            ni += __popc(m);
+            for (int q = 0; q < 4; ++q)
+              if (rem[q]) rem[q] = test(rem[q]);
           }
-          drain_items(false);
+          if (c > kPriv) { sm.kI[k] |= 0x8000u; c = 0; }  // too many candidates: slow path in D4
+          // pack the private lists: exclusive prefix of the counts
+          uint32_t pre = c;
+#pragma unroll
+          for (int d = 1; d < 32; d <<= 1) {
+            const uint32_t v = __shfl_up_sync(FULL, pre, d);
+            if (lane >= (uint32_t)d) pre += v;
+          }
+          const uint32_t tot = __shfl_sync(FULL, pre, 31);
+          pre -= c;
+          const uint32_t mc = __reduce_max_sync(FULL, c);
+          if (np + tot > 256u) drain_pairs(true);  // the pair list holds 256
+          __syncwarp();
+          for (uint32_t i = 0; i < mc; ++i)
+            if (i < c) sts_addr(a_pairs + 4u * (np + pre + i), k | (lds_u16_addr(a_priv + 2u * i) << 8));
+          np += tot;
+          drain_pairs(false);
         }
-        drain_items(true);
+        drain_pairs(true);
         __syncwarp();
-        // ---- D4: middle hits with candidates in both layers -> exact tests
-        uint32_t nj = 0;  // their numbers, compacted into sm.items
+        // ---- D4: middle hits with compatible hits in both layers -> exact (h0, h2) tests
+        uint32_t nj = 0;  // their numbers, compacted into the pair list's memory
         for (uint32_t kb = 0; kb < nk; kb += 32) {
           const uint32_t k = kb + lane;
           bool both = false;
           if (k < nk) {
-            const uint2 s02 = *reinterpret_cast<const uint2*>(&sm.occ[0][0] + 2 * k);
-            both = (s02.x >> 27) != 0 && (s02.y >> 27) != 0;
+            const uint2 s02 = *reinterpret_cast<const uint2*>(&sm.slot[2 * k]);
+            both = ((s02.x >> 27) != 0 && (s02.y >> 27) != 0) || (sm.kI[k] & 0x8000u);
           }
-#ifdef ST_DEBUG
-          {
-            uint32_t cc_ = 0, c4_ = 0;
-            if (k < nk) { const uint2 s02 = *reinterpret_cast<const uint2*>(&sm.occ[0][0] + 2 * k); cc_ = (s02.x >> 27) + (s02.y >> 27); c4_ = ((s02.x >> 27) > 3) + ((s02.y >> 27) > 3); }
-            ST_DBG(9, __reduce_add_sync(FULL, cc_)); ST_DBG(10, __reduce_add_sync(FULL, c4_));
-          }
-#endif
           const uint32_t m = __ballot_sync(FULL, both);
-          if (both) sm.items[nj + __popc(m & lt)] = k;
+          if (both) sts_addr(a_pairs + 4u * (nj + __popc(m & lt)), k);
           nj += __popc(m);
         }
-        __syncwarp();
-        const int64_t T01 = p.thr_in[s][0], T02 = p.thr_in[s][1], T12 = p.thr_in[s][2];
-        const uint64_t T01x2 = p.thr2_in[s][0], T02x2 = p.thr2_in[s][1], T12x2 = p.thr2_in[s][2];
         ST_DBG(4, nj);
+        __syncwarp();
         for (uint32_t jb = 0; jb < nj; jb += 32) {
-          uint32_t t = 0, i1 = 0, c0 = 0, c2 = 0, s0 = 0, s2w = 0;
+          uint32_t t = 0, i1 = 0;
           bool slow = false;
-          int32_t x1 = 0, y1 = 0;
           if (jb + lane < nj) {
-            const uint32_t k = sm.items[jb + lane];
-            const uint2 s02 = *reinterpret_cast<const uint2*>(&sm.occ[0][0] + 2 * k);
-            s0 = s02.x; s2w = s02.y;
-            c0 = s0 >> 27; c2 = s2w >> 27;
+            const uint32_t k = lds_addr(a_pairs + 4u * (jb + lane));
+            const uint2 s02 = *reinterpret_cast<const uint2*>(&sm.slot[2 * k]);
+            const uint32_t c0 = s02.x >> 27, c2 = s02.y >> 27;
             i1 = sm.kI[k];
-            slow = c0 > kSlotCap || c2 > kSlotCap;
-            if (slow) c0 = c2 = 0;
-            x1 = __ldg(x + b1 + i1); y1 = __ldg(y + b1 + i1);
-          }
-          const uint32_t mc0 = __reduce_max_sync(FULL, c0), mc2 = __reduce_max_sync(FULL, c2);
-          ST_DBG(5, mc0); ST_DBG(6, mc2); ST_DBG(7, __popc(__ballot_sync(FULL, slow))); ST_DBG(8, __reduce_add_sync(FULL, c0 + c2));
-          // h2 compatible with h1:  |x2*z1 - x1*z2| <= T12
-          int32_t x2[kSlotCap], y2[kSlotCap];
-          bool ok2[kSlotCap];
-          {
-            const int64_t Qx = anchor_q(x1, -z2, T12), Qy = anchor_q(y1, -z2, T12);
+            slow = c0 > 3u || c2 > 3u || (i1 & 0x8000u);
+            i1 &= 0x7FFFu;
+            if (!slow) {
+              // |x2*z0 - x0*z2| <= T02 for the <= 3 x 3 pairs (h0, h2), both already compatible with h1
+              int32_t x2[3] = {0, 0, 0}, y2[3] = {0, 0, 0};
 #pragma unroll
-            for (uint32_t b = 0; b < kSlotCap; ++b) {
-              x2[b] = 0; y2[b] = 0; ok2[b] = false;
-              if (b < mc2) {
-                if (b < c2) {
-                  const uint32_t j2 = ((s2w >> (9 * b)) & 0x1FFu) - 1u;
+              for (int b = 0; b < 3; ++b)
+                if ((uint32_t)b < c2) {
+                  const uint32_t j2 = ((s02.y >> (9 * b)) & 0x1FFu) - 1u;
                   x2[b] = __ldg(x + g2 + j2); y2[b] = __ldg(y + g2 + j2);
-                  ok2[b] = win_q(x2[b], z1, Qx, T12x2) & win_q(y2[b], z1, Qy, T12x2);
                 }
-              }
-            }
-          }
-          {
-            const int64_t Qx = anchor_q(x1, -z0, T01), Qy = anchor_q(y1, -z0, T01);
-            for (uint32_t a = 0; a < mc0; ++a) {
-              if (a < c0) {
-                const uint32_t j0 = ((s0 >> (9 * a)) & 0x1FFu) - 1u;
-                const int32_t x0 = __ldg(x + g0 + j0), y0 = __ldg(y + g0 + j0);
-                // h0 with h1: |x0*z1 - x1*z0| <= T01;  h2 with h0: |x2*z0 - x0*z2| <= T02
-                if (win_q(x0, z1, Qx, T01x2) & win_q(y0, z1, Qy, T01x2)) {
-                  const int64_t Px = anchor_q(x0, -z2, T02), Py = anchor_q(y0, -z2, T02);
+              int32_t x0[3] = {0, 0, 0}, y0[3] = {0, 0, 0};
 #pragma unroll
-                  for (uint32_t b = 0; b < kSlotCap; ++b)
-                    if (ok2[b]) t += (win_q(x2[b], z0, Px, T02x2) & win_q(y2[b], z0, Py, T02x2)) ? 1u : 0u;
+              for (int a = 0; a < 3; ++a)
+                if ((uint32_t)a < c0) {
+                  const uint32_t j0 = ((s02.x >> (9 * a)) & 0x1FFu) - 1u;
+                  x0[a] = __ldg(x + g0 + j0); y0[a] = __ldg(y + g0 + j0);
                 }
-              }
+#pragma unroll
+              for (int a = 0; a < 3; ++a)
+                if ((uint32_t)a < c0) {
+                  const int64_t Px = anchor_q(x0[a], -z2, T02), Py = anchor_q(y0[a], -z2, T02);
+#pragma unroll
+                  for (int b = 0; b < 3; ++b)
+                    if ((uint32_t)b < c2) t += (win_q(x2[b], z0, Px, T02x2) & win_q(y2[b], z0, Py, T02x2)) ? 1u : 0u;
+                }
             }
           }
           uint32_t sm_ = __ballot_sync(FULL, slow);
-          while (sm_) {  // rare: more than kSlotCap candidates in a layer
+          ST_DBG(7, __popc(sm_));
+          while (sm_) {  // rare: more than two compatible hits in a layer, or more than kPriv candidates
             const int src = __ffs((int)sm_) - 1;
             sm_ &= sm_ - 1;
-            const int32_t xs1 = __shfl_sync(FULL, x1, src), ys1 = __shfl_sync(FULL, y1, src);
-            const uint32_t ts = station_triplets_slow(StationGeo{x, y, b0, b1, b2, n0, n1, n2, z0, z1, z2, T01, T02, T12}, xs1, ys1);
+            const uint32_t is = __shfl_sync(FULL, i1, src);
+            const uint32_t ts = station_triplets_slow(StationGeo{x, y, b0, b1, b2, n0, n1, n2, z0, z1, z2, T01, T02, T12},
+                                                      __ldg(x1p + is), __ldg(y1p + is));
             if ((int)lane == src) t = ts;
           }
           trip += t;

@@ -178,6 +178,43 @@ def test_layers_up_to_max_hits_per_layer():
     assert got[1][0] >= 2 and got[2][0] == 1
 
 
+@pytest.mark.parametrize("impl", ["station", "team"])
+def test_class_h_kernel_variants(impl, monkeypatch):
+    # class H also has a one-warp-per-station kernel (station.cuh) and the team kernel; the default is chain_kernel.
+    # The library reads CBM_TRIGGER_H_IMPL at cbm_trigger_create.
+    monkeypatch.setenv("CBM_TRIGGER_H_IMPL", impl)
+    rng = np.random.default_rng(23)
+    z = list(W.GEOMETRY_4)
+    # every combination passes (closed forms; the oracle's triplet lists would be too long): slots and lists overflow
+    cones = [A.narrow_cone_event(z, 200, rng, spread_units=3), A.narrow_cone_event(z, 130, rng)]
+    x, y, off = W.batch_from_layers(z, cones)
+    nt, nc, ac, st = gpu_select(z, x, y, off)
+    assert nt.tolist() == [[200**3] * 4, [130**3] * 4] and nc.tolist() == [2**32 - 1] * 2 and st["n_class"][2] == 2
+    ev = [big_uniform_event(z, [448] * 12, rng), big_uniform_event(z, [129] + [300] * 11, rng),
+          big_uniform_event(z, [300, 0, 300] + [200] * 9, rng),  # a station with an empty layer
+          big_uniform_event(z, [400, 130, 5, 448, 448, 1, 1, 1, 200, 2, 300, 2], rng)]
+    lay = big_uniform_event(z, [300] * 12, rng)                  # planted tracks in a class-H event
+    for l, h in enumerate(A.exact_line_hits(z, 123, -77)):
+        lay[l][17] = h
+    for l, h in enumerate(A.exact_line_hits(z, -200, 31)):
+        lay[l][299] = h
+    ev.append(lay)
+    cl = big_uniform_event(z, [200] * 12, rng)                   # 12 hits of every layer around one slope: many
+    for l in range(12):                                          # compatible hits per middle hit
+        for i in range(12):
+            cl[l][i] = (int(0.1 * z[l]) + int(rng.integers(-300, 301)), int(-0.2 * z[l]) + int(rng.integers(-300, 301)))
+    ev.append(cl)
+    x, y, off = W.batch_from_layers(z, ev)
+    got = gpu_select(z, x, y, off)
+    assert_same(got, oracle_of(z, x, y, off), impl + " hand-built")
+    assert got[3]["n_class"][2] == len(ev)
+    cfg = W.CONFIGS[3]
+    b = W.generate(cfg, n_events=40000)
+    got = gpu_select(cfg.layer_z, b.x, b.y, b.off, win_in=cfg.win_in, win_link=cfg.win_link, min_candidates=cfg.min_candidates)
+    g = oracle.geometry(cfg.layer_z, cfg.win_in, cfg.win_link, cfg.min_candidates)
+    assert_same(got, oracle_mt(g, b.x, b.y, b.off), impl + " config 3")
+
+
 def test_invalid_offsets_are_rejected_on_the_device():
     rng = np.random.default_rng(5)
     z = list(W.GEOMETRY_4)
