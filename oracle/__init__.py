@@ -7,6 +7,8 @@ helpers or tables); the product never routes through it.
     run(...)            -> oracle/cbm_oracle.c   (the definition as nested loops, int64)
     run_slope_sorted()  -> oracle/slope_sorted.c (independent sorted/multiplicity route; a pin)
     brute_force         -> oracle/brute_force.py (no short-circuit, explicit S-tuples; a pin)
+    selected, unpack_xy20, gather, filter_layers, build_events -> plain Python loops (the definitions of the list of
+                           selected events, the packed wire format, the gather, the input filter, the event building)
 """
 from __future__ import annotations
 
@@ -238,3 +240,21 @@ def filter_layers(xyz, ev_off, layer_z):
                     ys.append(rec[i][1])
             off.append(len(xs))
     return np.asarray(xs, dtype=np.int32), np.asarray(ys, dtype=np.int32), np.asarray(off, dtype=np.uint32)
+
+
+def build_events(t, t_gap):
+    """Event building from a free-streaming, time-ordered hit stream (section 8: the data acquisition
+    "will deliver free-streaming data not associated to single event by a hardware trigger ... the time measurement of
+    each hit must be considered"; the paper gives no rule, reading B9 fixes one): the records of a timeslice
+    come in stream order with an integer time stamp t[i]; record i opens a new event iff i == 0 or
+    t[i] - t[i-1] > t_gap.  An event is a maximal run of records without such a gap.  Written out as the plain loop it is.
+
+    Returns ev_off (uint32 [n_events + 1]): ev_off[k] = first record of event k, ev_off[n_events] = number of records
+    ([0] for an empty stream)."""
+    ts = [int(v) for v in np.asarray(t).ravel().tolist()]
+    gap = int(t_gap)
+    starts = []
+    for i in range(len(ts)):
+        if i == 0 or ts[i] - ts[i - 1] > gap:
+            starts.append(i)
+    return np.asarray(starts + [len(ts)], dtype=np.uint32)

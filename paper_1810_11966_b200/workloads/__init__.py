@@ -289,3 +289,22 @@ def full_setup_stream(batch: Batch, other_hits_per_event=400, seed=0, other_z=No
         rec[~is_much, 1] = rng.integers(-400_000, 400_001, size=o)
         rec[~is_much, 2] = other_z[rng.integers(0, other_z.size, size=o)]
     return xyz, ev_off.astype(np.uint32)
+
+
+def timed_stream(batch: Batch, other_hits_per_event=100, mean_dt=100, spread=8, seed=0):
+    """A free-streaming timeslice around a generated batch (input formatting only; free-streaming
+    data, every hit with a time measurement): the records of full_setup_stream() in their stream order, plus a time
+    stamp per record in ns: interaction e happens at T_e (exponential gaps of mean `mean_dt`: 100 ns = CBM's 10 MHz,
+    PAPER.md:23), its records lie at T_e + sorted uniform offsets in [0, spread].  Returns (xyz int32 [N][3],
+    t int32 [N] non-decreasing, ev_off uint32 [E + 1] of the interactions)."""
+    xyz, ev_off = full_setup_stream(batch, other_hits_per_event=other_hits_per_event, seed=seed)
+    rng = np.random.default_rng(seed + 1000)
+    E = batch.n_events
+    T = np.cumsum(rng.exponential(mean_dt, size=E)).astype(np.int64) + np.arange(E, dtype=np.int64)  # strictly increasing
+    t = np.empty(xyz.shape[0], dtype=np.int64)
+    for e in range(E):
+        a, b = int(ev_off[e]), int(ev_off[e + 1])
+        t[a:b] = T[e] + np.sort(rng.integers(0, spread + 1, size=b - a))
+    t = np.maximum.accumulate(t)  # interactions closer than `spread` overlap: the stream stays time-ordered
+    assert t.size == 0 or t[-1] < 2**31
+    return xyz, t.astype(np.int32), ev_off
