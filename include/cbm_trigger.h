@@ -200,6 +200,23 @@ int cbm_trigger_gather_device(cbm_trigger_t* h, uint32_t n_events, uint64_t n_hi
 int cbm_trigger_filter_device(cbm_trigger_t* h, uint32_t n_events, uint64_t n_records, const int32_t* d_xyz,
                               const uint32_t* d_ev_off, int32_t* d_out_x, int32_t* d_out_y, uint32_t* d_out_off, void* stream);
 
+/* Event building from a free-streaming, time-stamped hit stream (section 8: the
+ * data acquisition "will deliver free-streaming data not associated to single event by a hardware trigger ... not only
+ * the spatial coordinates, but also the time measurement of each hit must be considered").  The paper states no rule;
+ * DESIGN.md reading B9 fixes one: the records of a timeslice come in stream order, d_t[i] (DEVICE, int32, any unit,
+ * e.g. ns from the start of the timeslice) is the time stamp of record i -- the fourth coordinate of the records
+ * (x, y, z) of cbm_trigger_filter_device, kept as a container of its own.  Record i opens a new event
+ * iff i == 0 or d_t[i] - d_t[i-1] > t_gap (exact 64-bit difference; a record earlier than its predecessor never opens
+ * one: stream order rules); an event is a maximal run of records without such a gap, so interactions closer than t_gap
+ * pile up into one event.  Output: d_ev_off (DEVICE, room for n_records + 1 uint32): d_ev_off[k] = first record of
+ * event k, d_ev_off[*n_events] = n_records -- the d_ev_off argument of cbm_trigger_filter_device, whose output goes to
+ * cbm_trigger_run_device.  *n_events (HOST) = number of events built.  Blocks until the count is on the host (the next
+ * calls need it as an argument); n_records < 2^32; no atomics, the output is unique.  Scratch is allocated and freed
+ * on `stream` (cudaMallocAsync).  An event built from more than max_hits_per_layer hits in a layer is rejected by the
+ * selection like any other such event (CBM_ERR_RANGE). */
+int cbm_trigger_build_events_device(cbm_trigger_t* h, uint64_t n_records, const int32_t* d_t, uint32_t t_gap,
+                                    uint32_t* d_ev_off, uint32_t* n_events, void* stream);
+
 /* The paper's own selection, literally (section 3.2), on caller-owned DEVICE
  * arrays (layout and stream as cbm_trigger_run_device; geometry = the handle's layer_z):
  *   1. all triplets of the trigger station, one hit from each layer

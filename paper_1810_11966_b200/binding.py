@@ -25,7 +25,7 @@ EXPORTS = (
     "cbm_trigger_get_stats", "cbm_trigger_last_error", "cbm_trigger_version", "cbm_trigger_device_kernel_times",
     "cbm_trigger_fetch_selected", "cbm_trigger_select_device",
     "cbm_trigger_host_buffers_packed", "cbm_trigger_upload_events_packed", "cbm_trigger_msd_device", "cbm_trigger_gather_device",
-    "cbm_trigger_ubench", "cbm_trigger_filter_device",
+    "cbm_trigger_ubench", "cbm_trigger_filter_device", "cbm_trigger_build_events_device",
 )
 PROFILE_RING = 32
 # scheduler classes (csrc/cbm_trigger.cu, csrc/params.h), restated for bookkeeping in bench.py only
@@ -157,6 +157,8 @@ def load_library():
         lib.cbm_trigger_msd_device.argtypes = [vp, ctypes.POINTER(MsdParams), u32, u64, vp, vp, vp, vp, vp, vp]
         lib.cbm_trigger_filter_device.restype = i32
         lib.cbm_trigger_filter_device.argtypes = [vp, u32, u64, vp, vp, vp, vp, vp, vp]
+        lib.cbm_trigger_build_events_device.restype = i32
+        lib.cbm_trigger_build_events_device.argtypes = [vp, u64, vp, u32, vp, ctypes.POINTER(u32), vp]
         lib.cbm_trigger_ubench.restype = i32
         lib.cbm_trigger_ubench.argtypes = [vp, ctypes.POINTER(Ubench)]
         lib.cbm_trigger_get_stats.restype = i32
@@ -286,6 +288,13 @@ def cbm_trigger_filter_device(handle, n_events, n_records, d_xyz, d_ev_off, d_ou
     """d_* are raw device addresses (ints); stream is a cudaStream_t as int."""
     _check(load_library().cbm_trigger_filter_device(handle, n_events, n_records, d_xyz, d_ev_off, d_out_x, d_out_y, d_out_off,
                                                     stream), handle)
+
+
+def cbm_trigger_build_events_device(handle, n_records, d_t, t_gap, d_ev_off, stream=0) -> int:
+    """d_* are raw device addresses (ints); blocks; returns the number of events built."""
+    n = ctypes.c_uint32(0)
+    _check(load_library().cbm_trigger_build_events_device(handle, n_records, d_t, t_gap, d_ev_off, ctypes.byref(n), stream), handle)
+    return int(n.value)
 
 
 def cbm_trigger_ubench(handle) -> dict:
@@ -429,6 +438,12 @@ class Trigger:
         st = torch.cuda.current_stream().cuda_stream if stream is None else stream
         cbm_trigger_filter_device(self.handle, n_events, n_records, d_xyz.data_ptr(), d_ev_off.data_ptr(), d_ox.data_ptr(),
                                   d_oy.data_ptr(), d_ooff.data_ptr(), st)
+
+    def build_events_device(self, n_records, d_t, t_gap, d_ev_off, stream=None) -> int:
+        """Event building from time stamps on torch CUDA tensors; returns the number of events."""
+        import torch
+        st = torch.cuda.current_stream().cuda_stream if stream is None else stream
+        return cbm_trigger_build_events_device(self.handle, n_records, d_t.data_ptr(), t_gap, d_ev_off.data_ptr(), st)
 
     def ubench(self) -> dict:
         return cbm_trigger_ubench(self.handle)

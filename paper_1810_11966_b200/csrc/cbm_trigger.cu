@@ -28,6 +28,7 @@
 #include "msd.cuh"
 #include "ubench.cuh"
 #include "filter.cuh"
+#include "timeslice.cuh"
 
 namespace {
 
@@ -811,6 +812,41 @@ int cbm_trigger_filter_device(cbm_trigger_t* h, uint32_t n_events, uint64_t n_re
   scan_write_kernel<<<nb, kSelThreads, 0, st>>>(scr.d_fcnt, n, d_bsum, d_out_off);
   filter_scatter_kernel<<<n_events, kFilterThreads, 0, st>>>(fp, d_xyz, d_ev_off, n_events, (uint32_t)n_records, d_out_off, d_out_x, d_out_y);
   CBM_CUDA(h, cudaGetLastError());
+  return CBM_OK;
+}
+
+int cbm_trigger_build_events_device(cbm_trigger_t* h, uint64_t n_records, const int32_t* d_t, uint32_t t_gap, uint32_t* d_ev_off,
+                                    uint32_t* n_events, void* stream) {
+  if (!h) return CBM_ERR_INVALID_ARG;
+  if (!n_events || !d_ev_off || (n_records && !d_t)) return fail(h, CBM_ERR_INVALID_ARG, "pointers must not be NULL");
+  if (n_records >= (1ull << 32)) return fail(h, CBM_ERR_CAPACITY, "n_records must be < 2^32");
+  cudaStream_t st = (cudaStream_t)stream;
+  CBM_CUDA(h, cudaSetDevice(h->cfg.device));
+  *n_events = 0;
+  if (n_records == 0) {
+    CBM_CUDA(h, cudaMemsetAsync(d_ev_off, 0, sizeof(uint32_t), st));
+    CBM_CUDA(h, cudaStreamSynchronize(st));
+    return CBM_OK;
+  }
+  const uint32_t n = (uint32_t)n_records;
+  const uint32_t nb = (n + kSelEvents - 1) / kSelEvents;
+  // scratch of this call (stream-ordered allocation): the flags, the per-block counts of the compaction, the count
+  uint8_t* d_flag = nullptr;
+  uint32_t* d_cnt = nullptr;
+  CBM_CUDA(h, cudaMallocAsync((void**)&d_flag, ((size_t)n + 15) & ~(size_t)15, st));
+  cudaError_t e = cudaMallocAsync((void**)&d_cnt, ((size_t)nb + 2) * sizeof(uint32_t), st);
+  if (e != cudaSuccess) { cudaFreeAsync(d_flag, st); return fail(h, CBM_ERR_CUDA, "cudaMallocAsync: %s", cudaGetErrorString(e)); }
+  uint32_t* const d_n = d_cnt + nb + 1;
+  event_flag_kernel<<<(n + kFlagThreads - 1) / kFlagThreads, kFlagThreads, 0, st>>>(d_t, n, t_gap, d_flag);
+  select_count_kernel<<<nb, kSelThreads, 0, st>>>(d_flag, n, d_cnt);
+  select_write_kernel<<<nb, kSelThreads, 0, st>>>(d_flag, n, d_cnt, d_ev_off, d_n);
+  event_close_kernel<<<1, 1, 0, st>>>(d_ev_off, d_n, n);
+  e = cudaGetLastError();
+  if (e == cudaSuccess) e = cudaMemcpyAsync(n_events, d_n, sizeof(uint32_t), cudaMemcpyDeviceToHost, st);
+  cudaFreeAsync(d_flag, st);
+  cudaFreeAsync(d_cnt, st);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  if (e != cudaSuccess) return fail(h, CBM_ERR_CUDA, "event building: %s", cudaGetErrorString(e));
   return CBM_OK;
 }
 
