@@ -49,6 +49,14 @@ __device__ __forceinline__ void reds_or_a(uint32_t addr, uint32_t v) {
   asm volatile("red.shared.or.b32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
 }
 
+// per-station constants: filled into shared memory once per CTA, read back with 128-bit loads once per station and warp
+struct alignas(16) ChainStationConst {
+  int32_t z0, z1, z2, nz0, nz2;  // nz = -z
+  int32_t M0, M1, M2;
+  int64_t T01, T02, T12;
+  uint64_t T01x2, T02x2, T12x2;
+};
+
 template <int W, int CAP, int NC, int LISTCAP>
 struct ChainSmem {
   alignas(16) int32_t sx[3 * CAP + 8];        // the station as it lies in x[] (from the 16-byte boundary below its
@@ -61,6 +69,7 @@ struct ChainSmem {
   uint32_t wcnt[W];                           // survivors in each part
   int32_t ux[2][LISTCAP], uy[2][LISTCAP];     // middle hits with triplets of the previous / current station
   uint32_t uc[2][LISTCAP];                    // their multiplicities, then saturated chain counts c_s[u]
+  alignas(16) ChainStationConst sc[kMaxStations];
   uint32_t off[kMaxLayers + 1];
   unsigned long long acc[2];                  // triplets of the station (parity-buffered with the two below)
   uint32_t ucount[2];
@@ -75,13 +84,6 @@ __device__ __forceinline__ uint32_t chain_cell_of(int key, int sh, uint32_t mask
 
 
 
-// per-station constants, loaded once per station
-struct ChainStationConst {
-  int32_t z0, z1, z2, nz0, nz2;  // nz = -z
-  int32_t M0, M1, M2;
-  int64_t T01, T02, T12;
-  uint64_t T01x2, T02x2, T12x2;
-};
 
 // Chain heads (index + 1 <= 4096, 16 bits each) of the <= 2x2 coarse cells that can hold a hit compatible with
 // a hit whose window covers rows lox..hix and columns loy..hiy (cyclic); non-empty heads only, packed from bit 0.
@@ -151,6 +153,16 @@ __global__ void __launch_bounds__(32 * W, MINB)
     uint4* const v = reinterpret_cast<uint4*>(sm.head);
     for (uint32_t i = tid; i < kZeroVec; i += T) v[i] = make_uint4(0, 0, 0, 0);
   }
+  if (tid < S) {
+    const uint32_t t = tid;
+    ChainStationConst c;
+    c.z0 = p.z[3 * t]; c.z1 = p.z[3 * t + 1]; c.z2 = p.z[3 * t + 2];
+    c.nz0 = -c.z0; c.nz2 = -c.z2;
+    c.M0 = p.key_mul[3 * t]; c.M1 = p.key_mul[3 * t + 1]; c.M2 = p.key_mul[3 * t + 2];
+    c.T01 = p.thr_in[t][0]; c.T02 = p.thr_in[t][1]; c.T12 = p.thr_in[t][2];
+    c.T01x2 = p.thr2_in[t][0]; c.T02x2 = p.thr2_in[t][1]; c.T12x2 = p.thr2_in[t][2];
+    sm.sc[t] = c;
+  }
   if (tid == 0) {
     sm.li[0] = atomicAdd(&ctrl->work[CLS], 1u);
     sm.li[1] = atomicAdd(&ctrl->work[CLS], 1u);
@@ -202,12 +214,7 @@ __global__ void __launch_bounds__(32 * W, MINB)
       const uint32_t b0 = sm.off[3 * s], b1 = sm.off[3 * s + 1], b2 = sm.off[3 * s + 2], b3 = sm.off[3 * s + 3];
       const uint32_t n0 = b1 - b0, n1 = b2 - b1, n2 = b3 - b2;
       const uint32_t o0 = b0 & 3u, o1 = o0 + n0, o2 = o1 + n1;  // layer starts in sm.sx / sm.sy
-      ChainStationConst c;
-      c.z0 = p.z[3 * s]; c.z1 = p.z[3 * s + 1]; c.z2 = p.z[3 * s + 2];
-      c.nz0 = -c.z0; c.nz2 = -c.z2;
-      c.M0 = p.key_mul[3 * s]; c.M1 = p.key_mul[3 * s + 1]; c.M2 = p.key_mul[3 * s + 2];
-      c.T01 = p.thr_in[s][0]; c.T02 = p.thr_in[s][1]; c.T12 = p.thr_in[s][2];
-      c.T01x2 = p.thr2_in[s][0]; c.T02x2 = p.thr2_in[s][1]; c.T12x2 = p.thr2_in[s][2];
+      const ChainStationConst c = sm.sc[s];
       const bool search = (n0 != 0) & (n1 != 0) & (n2 != 0);
       const uint32_t vwarp = (warp + rot) & (W - 1), vtid = vwarp * 32 + lane;
       rot = (rot + 1u) & (W - 1);
@@ -339,7 +346,7 @@ __global__ void __launch_bounds__(32 * W, MINB)
                       q >>= 16;
                     } while (q);
                   } else {
-                    t += chain_count_h0_slow(sm, head0, o0, lox, hix, loy, hiy, nc, c, Qx, Qy, x2, y2);
+                    t += chain_count_h0_slow(sm, head0, o0, lox, hix, loy, hiy, nc, sm.sc[s], Qx, Qy, x2, y2);
                   }
                 }
                 cu = nx;
