@@ -85,6 +85,20 @@ def ncu_traffic(workload, kernel):
     return None
 
 
+def ncu_instructions(workload):
+    """smsp__inst_executed.sum of the committed `ncu --set full` captures of this workload's kernels
+    (profiles/r2_inst.csv names capture and commit): {kernel: warp-instructions per launch}."""
+    path = os.path.join(ROOT, "profiles/r2_inst.csv")
+    res = {}
+    if os.path.exists(path):
+        with open(path) as f:
+            for row in csv.DictReader(f):
+                if row.get("workload") == workload:
+                    res[row["kernel"]] = {"warp_instructions": int(row["warp_instructions"]), "capture": row.get("capture"),
+                                          "commit": row.get("commit")}
+    return res
+
+
 class ClockSampler:
     """nvidia-smi clocks and throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
 
@@ -457,6 +471,17 @@ def run_ours(args, cfg, cid):
                           "frac_of_8TBs_nominal": step_gbs / 8000.0, "algorithmic_bytes_per_step": B_alg, "t_hbm_ms": t_hbm_ms},
         "clocks": clocks, "warmup_steps_run": n_warm, "generation_s": t_gen,
     }
+    # What the kernels are bound by in fact: instruction issue.  The warp-instructions of the
+    # captured kernels of this workload (committed ncu captures) at one instruction per scheduler and cycle.
+    inst = ncu_instructions(cfg.name)
+    if inst and clocks.get("sm_mhz"):
+        n_sched = 4 * torch.cuda.get_device_properties(local_rank).multi_processor_count
+        wi = sum(v["warp_instructions"] for v in inst.values())
+        t_issue_ms = wi / (n_sched * clocks["sm_mhz"] * 1e6) * 1e3
+        out["roofline_step"]["issue"] = {
+            "warp_instructions_per_step": wi, "kernels": inst, "schedulers": n_sched, "sm_mhz": clocks["sm_mhz"],
+            "t_issue_ms": t_issue_ms, "frac": t_issue_ms / ms_per_step,
+            "note": "captured kernels only; the step cannot be shorter than t_issue_ms at this instruction count"}
     if ubench:
         out["ubench"] = dict(ubench, note="cbm_trigger_ubench: measured on this GPU in this run, 8 chains per thread")
     if e2e:
