@@ -877,7 +877,8 @@ int cbm_trigger_msd_device(cbm_trigger_t* h, const cbm_trigger_msd_params_t* mp,
   d.pre_x = delta(d.num_x, d.den_x) * ((int64_t)d.z0 + d.z1);
   d.pre_y = delta(d.num_y, d.den_y) * ((int64_t)d.z0 + d.z1);
   CBM_CUDA(h, cudaSetDevice(h->cfg.device));
-  msd_kernel<<<(n_events + kMsdWarps - 1) / kMsdWarps, 32 * kMsdWarps, 0, (cudaStream_t)stream>>>(
+  constexpr uint32_t kMsdEventsPerCta = kMsdWarps * 32 / kMsdLanes;
+  msd_kernel<<<(n_events + kMsdEventsPerCta - 1) / kMsdEventsPerCta, 32 * kMsdWarps, 0, (cudaStream_t)stream>>>(
       d, d_x, d_y, d_off, n_events, (uint32_t)n_hits, d_n_passing, d_accept);
   CBM_CUDA(h, cudaGetLastError());
   return CBM_OK;

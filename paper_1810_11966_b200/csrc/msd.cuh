@@ -9,7 +9,7 @@
 // 128-bit integers; exact for any int32 coordinates and 0 < z <= 2^23 (Svz < 2^56 in int64, Svv < 2^64 in uint64,
 // Szz*Svv < 2^112, left side < 2^124, right side < 2^92).
 //
-// One warp per event; lane <-> (h0,h1) pair.  A passing triplet has every residual |r_i| <= delta = sqrt(thr*ndf),
+// Sixteen lanes per event (two events per warp); lane <-> hit of layer 0, loop over layer 1.  A passing triplet has every residual |r_i| <= delta = sqrt(thr*ndf),
 // hence |v1*z0 - v0*z1| = |r1*z0 - r0*z1| <= delta*(z0+z1): an exact 64-bit necessary condition on the pair that
 // keeps the 128-bit test and the h2 loop for the few pairs that can belong to a passing triplet.
 #pragma once
@@ -26,6 +26,7 @@ struct MsdDev {
 };
 
 constexpr int kMsdWarps = 4;
+constexpr int kMsdLanes = 16;  // lanes per event: the paper's trigger station holds about 15 hits per layer
 
 __device__ __forceinline__ bool msd_ok(int64_t v0, int64_t v1, int64_t v2, int64_t z0, int64_t z1, int64_t z2, int64_t szz,
                                        uint32_t num, uint32_t den, uint32_t ndf) {
@@ -41,36 +42,39 @@ __device__ __forceinline__ bool msd_ok(int64_t v0, int64_t v1, int64_t v2, int64
 __global__ void __launch_bounds__(32 * kMsdWarps)
     msd_kernel(const MsdDev p, const int32_t* __restrict__ x, const int32_t* __restrict__ y, const uint32_t* __restrict__ off,
                uint32_t n_events, uint32_t n_hits, uint32_t* __restrict__ n_passing, uint8_t* __restrict__ accept) {
-  const uint32_t lane = threadIdx.x & 31;
-  const uint32_t e = blockIdx.x * kMsdWarps + (threadIdx.x >> 5);
-  if (e >= n_events) return;
+  const uint32_t lane = threadIdx.x & (kMsdLanes - 1);
+  const uint32_t e = blockIdx.x * (kMsdWarps * 32 / kMsdLanes) + threadIdx.x / kMsdLanes;
+  if (e >= n_events) return;  // whole groups of kMsdLanes lanes leave: the shuffles below stay inside a group
   const uint32_t* o = off + (size_t)e * p.L + p.first_layer;
   const uint32_t o0 = __ldg(o), o1 = __ldg(o + 1), o2 = __ldg(o + 2), o3 = __ldg(o + 3);
   unsigned long long cnt = 0;
   const bool well_formed = (o0 <= o1) & (o1 <= o2) & (o2 <= o3) & (o3 <= n_hits);
   if (well_formed) {  // a malformed event selects nothing and is never accepted
-    const uint32_t n1 = o2 - o1;
-    const unsigned long long n_pairs = (unsigned long long)(o1 - o0) * n1;
     const int64_t z0 = p.z0, z1 = p.z1, z2 = p.z2;
     const int64_t szz = z0 * z0 + z1 * z1 + z2 * z2;
-    for (unsigned long long q = lane; q < n_pairs; q += 32) {
-      const uint32_t i0 = (uint32_t)(q / n1), i1 = (uint32_t)(q - (unsigned long long)i0 * n1);
-      const int64_t x0 = __ldg(x + o0 + i0), x1 = __ldg(x + o1 + i1);
-      const int64_t dx = x1 * z0 - x0 * z1;
-      if ((dx < 0 ? -dx : dx) > p.pre_x) continue;
-      const int64_t y0 = __ldg(y + o0 + i0), y1 = __ldg(y + o1 + i1);
-      const int64_t dy = y1 * z0 - y0 * z1;
-      if ((dy < 0 ? -dy : dy) > p.pre_y) continue;
-      for (uint32_t i2 = o2; i2 < o3; ++i2) {
-        const int64_t x2 = __ldg(x + i2), y2 = __ldg(y + i2);
-        if (msd_ok(x0, x1, x2, z0, z1, z2, szz, p.num_x, p.den_x, p.ndf) &&
-            msd_ok(y0, y1, y2, z0, z1, z2, szz, p.num_y, p.den_y, p.ndf))
-          ++cnt;
+    // lane <-> hit of layer 0; the hits of layers 1 and 2 are read at addresses uniform in the group (one transaction each)
+    for (uint32_t i0 = o0 + lane; i0 < o1; i0 += kMsdLanes) {
+      const int64_t x0 = __ldg(x + i0), y0 = __ldg(y + i0);
+      const int64_t ax = x0 * z1, ay = y0 * z1;
+      for (uint32_t i1 = o1; i1 < o2; ++i1) {
+        const int64_t x1 = __ldg(x + i1);
+        const int64_t dx = x1 * z0 - ax;
+        if ((dx < 0 ? -dx : dx) > p.pre_x) continue;  // exact necessary condition on the pair (h0, h1)
+        const int64_t y1 = __ldg(y + i1);
+        const int64_t dy = y1 * z0 - ay;
+        if ((dy < 0 ? -dy : dy) > p.pre_y) continue;
+        for (uint32_t i2 = o2; i2 < o3; ++i2) {
+          const int64_t x2 = __ldg(x + i2), y2 = __ldg(y + i2);
+          if (msd_ok(x0, x1, x2, z0, z1, z2, szz, p.num_x, p.den_x, p.ndf) &&
+              msd_ok(y0, y1, y2, z0, z1, z2, szz, p.num_y, p.den_y, p.ndf))
+            ++cnt;
+        }
       }
     }
   }
+  const uint32_t gmask = kMsdLanes == 32 ? 0xFFFFFFFFu : (((1u << kMsdLanes) - 1u) << ((threadIdx.x & 31u) & ~(uint32_t)(kMsdLanes - 1)));
 #pragma unroll
-  for (int d = 16; d >= 1; d >>= 1) cnt += __shfl_xor_sync(0xFFFFFFFFu, cnt, d);
+  for (int d = kMsdLanes / 2; d >= 1; d >>= 1) cnt += __shfl_xor_sync(gmask, cnt, d);
   if (lane == 0) {
     const uint32_t c = cnt > 0xFFFFFFFFull ? 0xFFFFFFFFu : (uint32_t)cnt;
     n_passing[e] = c;
