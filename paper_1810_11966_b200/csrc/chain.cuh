@@ -73,6 +73,7 @@ struct ChainSmem {
   uint32_t off[kMaxLayers + 1];
   unsigned long long acc[2];                  // triplets of the station (parity-buffered with the two below)
   uint32_t ucount[2];
+  uint32_t alive[2];                          // some chain count of the station is not zero (parity-buffered)
   uint32_t li[3];                             // ring of fetched work indices
   alignas(8) uint64_t bar;                    // completion of the station's bulk copies
 };
@@ -168,6 +169,7 @@ __global__ void __launch_bounds__(32 * W, MINB)
     sm.li[1] = atomicAdd(&ctrl->work[CLS], 1u);
     sm.acc[0] = sm.acc[1] = 0;
     sm.ucount[0] = sm.ucount[1] = 0;
+    sm.alive[0] = sm.alive[1] = 0;
     mbar_init(&sm.bar, 1);
     fence_mbar_init();
   }
@@ -387,11 +389,14 @@ __global__ void __launch_bounds__(32 * W, MINB)
         n_triplets[(size_t)e * S + s] = sat32(sm.acc[sp]);
         sm.acc[sp ^ 1u] = 0;
         sm.ucount[sp ^ 1u] = 0;
+        sm.alive[sp ^ 1u] = 0;
         if (s + 1 < S && searchable(s + 1)) issue_stage(s + 1);
       }
       if (search) {
         uint4* const v = reinterpret_cast<uint4*>(sm.head);
-        for (uint32_t i = tid; i < kZeroVec; i += T) v[i] = make_uint4(0, 0, 0, 0);
+#pragma unroll
+        for (uint32_t k = 0; k < (kZeroVec + T - 1) / T; ++k)  // straight-line: kZeroVec / T stores per thread
+          if ((k + 1) * T <= kZeroVec || tid + k * T < kZeroVec) v[tid + k * T] = make_uint4(0, 0, 0, 0);
       }
       if (s == 0 && pf_b > pf_a) {  // pull the next event of this team into L2 while this one is being searched
         const uint32_t la = pf_a >> 5, lb = (pf_b + 31) >> 5;  // 128-byte lines
@@ -422,7 +427,11 @@ __global__ void __launch_bounds__(32 * W, MINB)
             }
 #pragma unroll
             for (int d = kLinkG / 2; d >= 1; d >>= 1) a += __shfl_xor_sync(FULL, a, d);
-            if (u < ncur && g == 0) sm.uc[cur][u] = sat32((unsigned long long)sat32(a) * sm.uc[cur][u]);  // m_u <= 2^24
+            if (u < ncur && g == 0) {
+              const uint32_t v = sat32((unsigned long long)sat32(a) * sm.uc[cur][u]);  // m_u <= 2^24
+              sm.uc[cur][u] = v;
+              if (v) sm.alive[sp] = 1;
+            }
           }
         } else {  // rare: some entries live in the global spill area
           auto LX = [&](int w, uint32_t i) { return i < (uint32_t)LISTCAP ? sm.ux[w][i] : spill_i[(w * 3 + 0) * CAP + i - LISTCAP]; };
@@ -437,6 +446,7 @@ __global__ void __launch_bounds__(32 * W, MINB)
             }
             const uint32_t v = sat32((unsigned long long)sat32(a) * LC(cur, u));
             if (u < (uint32_t)LISTCAP) sm.uc[cur][u] = v; else spill_cta[(cur * 3 + 2) * CAP + u - LISTCAP] = v;
+            if (v) sm.alive[sp] = 1;
           }
         }
       }
@@ -445,6 +455,9 @@ __global__ void __launch_bounds__(32 * W, MINB)
       cur ^= 1;
       sp ^= 1u;
       team_sync<W>();
+      // every chain ends here (all c_s[u] are zero): no candidate, whatever the later stations hold; they are still
+      // searched for their triplet counts, but build no lists and link nothing
+      if (s > 0 && !dead && sm.alive[sp ^ 1u] == 0) dead = true;
     }
 
     // ---- candidates = sum over the last station's middle hits; a8: one writer per event
