@@ -2,7 +2,8 @@
 // still the fastest on; team.cuh holds the design used for classes M, G and list X).
 //
 // One team = one CTA of W warps works on one event at a time (persistent: events are fetched from the class list
-// with an atomic cursor, two fetches ahead so that the next event can be prefetched into L2).
+// with an atomic cursor, two fetches ahead).  An L2 prefetch of the next event was measured and dropped: it re-read 17 %
+// of the bytes from DRAM and did not shorten the kernel.
 // CAP = fullest layer the class admits; NC = coarse cells per axis the shared-memory tables are sized for;
 // LISTCAP = middle hits with triplets kept in shared memory per station (more spill to a global scratch).
 //
@@ -195,16 +196,8 @@ __global__ void __launch_bounds__(32 * W, MINB)
   for (uint32_t it3 = 0;; it3 = it3 == 2 ? 0 : it3 + 1) {
     const uint32_t li = sm.li[it3];
     if (li >= n_list) break;
-    const uint32_t nxt = sm.li[it3 == 2 ? 0 : it3 + 1];
     if (tid == 0) sm.li[it3 == 0 ? 2 : it3 - 1] = atomicAdd(&ctrl->work[CLS], 1u);
     const uint32_t e = __ldg(list + li);
-    // extent of the NEXT event: loaded now, used for its L2 prefetch during station 0 (latency hidden)
-    uint32_t pf_a = 0, pf_b = 0;
-    if (nxt < n_list) {
-      const uint32_t e2 = __ldg(list + nxt);
-      pf_a = __ldg(off + (size_t)e2 * L);
-      pf_b = __ldg(off + (size_t)e2 * L + L);
-    }
     for (uint32_t i = tid; i <= L; i += T) sm.off[i] = __ldg(off + (size_t)e * L + i);
     team_sync<W>();
     if (tid == 0 && searchable(0)) issue_stage(0);
@@ -397,13 +390,6 @@ __global__ void __launch_bounds__(32 * W, MINB)
 #pragma unroll
         for (uint32_t k = 0; k < (kZeroVec + T - 1) / T; ++k)  // straight-line: kZeroVec / T stores per thread
           if ((k + 1) * T <= kZeroVec || tid + k * T < kZeroVec) v[tid + k * T] = make_uint4(0, 0, 0, 0);
-      }
-      if (s == 0 && pf_b > pf_a) {  // pull the next event of this team into L2 while this one is being searched
-        const uint32_t la = pf_a >> 5, lb = (pf_b + 31) >> 5;  // 128-byte lines
-        for (uint32_t l = la + tid; l < lb; l += T) {
-          prefetch_l2(x + (size_t)l * 32);
-          prefetch_l2(y + (size_t)l * 32);
-        }
       }
       // ---- a7: chain counts c_s[u] = m_u * sum over linked t of c_{s-1}[t], saturating (R9)
       if (s > 0 && ncur) {
