@@ -40,7 +40,7 @@ using SmemM = TeamSmem<1, 128, 64, 4, 4, 32>;
 using SmemH = TeamSmem<4, 448, 192, 5, 5, 48>;
 using SmemG = TeamSmem<16, 4096, 4104, 5, 5, 256>;
 constexpr int kCapM = SmemM::CAP, kCapH = SmemH::CAP, kCapG = SmemG::CAP;
-constexpr int kMinBM = 24, kMinBH = 9, kMinBG = 1;
+constexpr int kMinBM = 24, kMinBH = 9, kMinBG = 2;
 #define TEAM_KERNEL_M team_kernel<SmemM, kClsM, kMinBM, false, true>
 #define TEAM_KERNEL_H team_kernel<SmemH, kClsH, kMinBH, false, true>
 // class H, round-1 design (chain.cuh): 4 warps, 448 hits per layer, 32 x 32 coarse cells, 64 list entries, 8 CTAs/SM
