@@ -378,11 +378,14 @@ int launch_selection(cbm_trigger* h, const Scratch& scr, const int32_t* d_x, con
       p, d_x, d_y, d_off, d_nt, d_nc, d_ac, scr.d_ctrl, scr.d_list[kClsM], scr.d_list[kClsX], nullptr);
   CBM_CUDA(h, rec(kKTeamM, 1, s_m));
   CBM_CUDA(h, rec(kKTeamH, 0, st));
-  if (h->h_impl == 0)
+  if (h->h_impl == 0) {
+    // the per-event station counters reset themselves at the end of a run; cleared here too, so that a run that was
+    // cut short cannot leave a count behind
+    CBM_CUDA(h, cudaMemsetAsync(scr.d_done, 0, (size_t)n_events * sizeof(uint32_t), st));
     STATION_KERNEL_H<<<h->grid_hs, 32 * kStWarps, kStWarps * sizeof(SmemHS), st>>>(
         p, d_x, d_y, d_off, d_nt, d_nc, d_ac, scr.d_ctrl, scr.d_list[kClsH], scr.d_list[kClsX], scr.d_st_cnt, scr.d_st_ent,
         scr.d_done);
-  else if (h->h_impl == 1)
+  } else if (h->h_impl == 1)
     CHAIN_KERNEL_H<<<h->grid_hc, 32 * SmemH::W, 0, st>>>(p, d_x, d_y, d_off, d_nt, d_nc, d_ac, scr.d_ctrl, scr.d_list[kClsH],
                                                         scr.d_spill[2]);
   else
