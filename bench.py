@@ -15,6 +15,8 @@ is stated on.
                max(t_HBM, t_INT), t_INT from the measured window-evaluation rate (cbm_trigger_ubench) and the
                oracle-side N_eval of a sample
   cpu_baseline the CPU oracle on the host cores (all cores, and one core)
+  config4_streaming  (default run only) the key figures of `--config 4`, run in a process of its own: a ring of
+               three distinct 10^6-event chunks, ten chunk-iterations, int32 and packed wire format, against 10 MHz
 
 Prints ONE JSON line (rank 0).  `--impl reference` times the CPU oracle (oracle/) on the host cores.
 """
@@ -56,6 +58,9 @@ def parse_args():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-packed", action="store_true", help="skip the end-to-end leg with the packed wire format XY20")
     ap.add_argument("--no-ubench", action="store_true", help="skip the integer-pipe micro-benchmarks")
+    ap.add_argument("--no-caller-memory", action="store_true", help="skip the end-to-end leg from pageable caller arrays")
+    ap.add_argument("--no-streaming-leg", action="store_true",
+                    help="default run (config 3, 1 GPU): do not add the streaming configuration (config 4) to the line")
     ap.add_argument("--serial", action="store_true", help="CBM_FLAG_SERIAL also in the timed leg (kernels one after the other)")
     return ap.parse_args()
 
@@ -415,7 +420,7 @@ def run_ours(args, cfg, cid):
         e2e = run_e2e(args, cfg, batch, ref, K, W, local_rank, rank, barrier)
         if not args.no_packed and world == 1:
             e2e_packed = run_e2e(args, cfg, batch, ref, K, W, local_rank, rank, barrier, packed=True)
-        if world == 1:
+        if world == 1 and not args.no_caller_memory:
             e2e_caller = run_e2e(args, cfg, batch, ref, K, W, local_rank, rank, barrier, caller_memory=True)
     del dx, dy, doff
 
@@ -519,7 +524,7 @@ def run_ours(args, cfg, cid):
             rs["t_int_ms_at_measured_window_rate"] = nev * E / ubench["window_evals_per_s"] * 1e3
             rs["bound"] = "hbm" if t_hbm_ms >= t_int_ms else "alu"
             rs["frac_of_stated_roofline"] = max(t_hbm_ms, t_int_ms) / ms_per_step
-    print(json.dumps(out))
+    return out
 
 
 def run_e2e(args, cfg, batch, ref, K, W, local_rank, rank, barrier, packed=False, caller_memory=False):
@@ -687,7 +692,41 @@ def main():
     elif args.mode == "msd":
         run_msd(args)
     else:
-        run_ours(args, cfg, args.config)
+        out = run_ours(args, cfg, args.config)
+        if out is None:  # not rank 0
+            return
+        if args.config == 3 and out["n_gpus"] == 1 and not args.no_streaming_leg and not args.no_e2e:
+            out["config4_streaming"] = streaming_leg()
+        print(json.dumps(out))
+
+
+def streaming_leg():
+    """BASELINE.json configs[4] beside the default line (config 3 carries the roofline target, config 4 the sustained
+    rate against 10 MHz): this script again with --config 4 in a process of its own -- a ring of three distinct
+    10^6-event chunks of seed 5, ten chunk-iterations, int32 and packed wire format, results of every slot compared
+    with device-resident results -- and the key figures of its line."""
+    import subprocess
+    cmd = [sys.executable, os.path.abspath(__file__), "--config", "4", "--steps", "10", "--warmup", "3", "--no-cpu-baseline",
+           "--no-ubench", "--no-caller-memory"]
+    try:
+        r = subprocess.run(cmd, capture_output=True, text=True, timeout=900)
+        line = [l for l in r.stdout.strip().splitlines() if l.startswith("{")][-1]
+        d = json.loads(line)
+    except Exception as ex:  # the default line must survive a failure of the extra leg
+        return {"error": f"{type(ex).__name__}: {ex}"}
+    keep = {"workload": d["config"]["workload"], "events_per_chunk": d["config"]["events_per_batch"],
+            "hits_per_chunk": d["config"]["hits_per_batch"], "value_hbm_resident": d["value"], "ms_per_step": d["ms_per_step"],
+            "roofline_step_frac": d["roofline_step"]["frac"], "kernels_ms": {k: v["ms"] for k, v in d["kernels"].items()},
+            "clocks": d.get("clocks")}
+    for k in ("e2e", "e2e_packed_xy20"):
+        if k in d:
+            keep[k] = d[k]
+    if "e2e" in d:
+        keep["sustained_value"] = d["e2e"]["value"]
+        keep["sustained_vs_10MHz"] = d["e2e"]["vs_10MHz"]
+    if "e2e_packed_xy20" in d:
+        keep["sustained_packed_vs_10MHz"] = d["e2e_packed_xy20"]["vs_10MHz"]
+    return keep
 
 
 if __name__ == "__main__":
