@@ -2,7 +2,7 @@
 //
 // Owns the slots (pinned host staging, device arrays, result buffers), the three streams of the
 // H2D | kernels | D2H software pipeline ("it can be hidden by performing computation and
-// transfer in parallel") and the launch sequence of the kernels in kernels.cuh.  No CPU fallback exists:
+// transfer in parallel") and the launch sequence of the kernels (classify, tile, team, chain, station .cuh).  No CPU fallback exists:
 // without a CUDA device cbm_trigger_create fails with CBM_ERR_CUDA.
 #include <cuda_runtime.h>
 
