@@ -171,6 +171,42 @@ int cbm_trigger_fetch_selected(cbm_trigger_t* h, uint32_t slot, uint32_t* event_
 int cbm_trigger_select_device(cbm_trigger_t* h, uint32_t n_events, const uint8_t* d_accept, uint32_t* d_event_ids,
                               uint32_t* d_n_selected, void* stream);
 
+/* The list of selected events for callers that must not allocate device memory.
+ *
+ * Who needs it: a readout node that runs the selection inside its data-taking loop.  Such a node hands out all of its
+ * device memory once, at start of run (timeslice buffers, result rings), and from then on nothing in the loop may call
+ * cudaMalloc / cudaFree: both stall every stream of the device until they return, which breaks the overlap of
+ * transfer and computation the loop lives on, and on a card that is fully handed out they simply fail.
+ * The same holds for code that is plugged into somebody else's framework and only receives device pointers and a
+ * stream from it.  Every other entry point of this library needs a handle, and cbm_trigger_create allocates.  This one
+ * takes no handle and allocates nothing, neither on the device nor on the host, neither here nor in a library routine.
+ *
+ * What it does: exactly cbm_trigger_select_device -- d_accept[n_events] uint8 in; out: d_event_ids
+ * (room for n_events uint32) = the ids of the events with accept != 0, ascending, and *d_n_selected (one uint32) =
+ * their number; all three DEVICE, owned by the caller; elements of d_event_ids beyond the count are left alone.  It
+ * runs on the calling thread's CURRENT device, on `stream` (a cudaStream_t of that device passed as void*; NULL = the
+ * legacy default stream), and returns without waiting.
+ *
+ * The price: the per-block counts of the compaction live in one fixed array inside the library's device image
+ * (CBM_TRIGGER_NOALLOC_MAX_EVENTS / 4096 uint32 = 16 KB).  Every GPU that loads the library carries these 16 KB until
+ * the process ends, whether the call is used or not.  n_events above CBM_TRIGGER_NOALLOC_MAX_EVENTS is refused with
+ * CBM_ERR_CAPACITY before anything is enqueued (split the batch, or use a handle).
+ * There is one such array per device and every call on that device uses it.  Nothing in it has to be zero at the
+ * start: each call first writes every entry it later reads, so the previous call's contents do no harm.  But two calls
+ * that run on the GPU at the same time (different streams without an event between them, or two host threads) overwrite
+ * each other's counts and both results are garbage: order the calls on one device yourself.  Calls on different
+ * devices are independent.
+ *
+ * First call on a device: it looks up where the driver put the array on that device and keeps the address (host
+ * side, a few bytes, under a lock); with lazy module loading this is also when the driver brings the two kernels onto
+ * the device.  Make that first call during set-up, outside any stream capture; later calls only launch kernels.
+ *
+ * Errors (message from cbm_trigger_last_error(NULL), per thread): CBM_ERR_INVALID_ARG for a NULL pointer,
+ * CBM_ERR_CAPACITY as above, CBM_ERR_CUDA if the device lookup or a launch fails.  Nothing is enqueued on error. */
+#define CBM_TRIGGER_NOALLOC_MAX_EVENTS (1u << 24)
+int cbm_trigger_select_noalloc(uint32_t n_events, const uint8_t* d_accept, uint32_t* d_event_ids, uint32_t* d_n_selected,
+                               void* stream);
+
 /* The hits of the selected events as a compact batch (the selected events go
  * on to full track reconstruction), on caller-owned DEVICE arrays on the caller's stream.  In: the batch
  * (d_x, d_y, d_off as in cbm_trigger_run_device) and the list from cbm_trigger_select_device (d_event_ids,
@@ -280,7 +316,7 @@ int cbm_trigger_ubench(cbm_trigger_t* h, cbm_trigger_ubench_t* out);
 int cbm_trigger_get_stats(cbm_trigger_t* h, uint32_t slot, cbm_trigger_stats_t* stats);
 
 /* Handle-owned, NUL-terminated message of the last failing call ("" if none).  With h == NULL: the message of
- * the last failing cbm_trigger_create on this thread. */
+ * the last failing cbm_trigger_create or cbm_trigger_select_noalloc on this thread. */
 const char* cbm_trigger_last_error(const cbm_trigger_t* h);
 
 /* "cbm-trigger <version> sm_100a" */

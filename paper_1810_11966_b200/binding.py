@@ -23,7 +23,7 @@ EXPORTS = (
     "cbm_trigger_create", "cbm_trigger_destroy", "cbm_trigger_host_buffers", "cbm_trigger_upload_events",
     "cbm_trigger_run", "cbm_trigger_fetch_results", "cbm_trigger_run_device", "cbm_trigger_device_status",
     "cbm_trigger_get_stats", "cbm_trigger_last_error", "cbm_trigger_version", "cbm_trigger_device_kernel_times",
-    "cbm_trigger_fetch_selected", "cbm_trigger_select_device",
+    "cbm_trigger_fetch_selected", "cbm_trigger_select_device", "cbm_trigger_select_noalloc",
     "cbm_trigger_host_buffers_packed", "cbm_trigger_upload_events_packed", "cbm_trigger_msd_device", "cbm_trigger_gather_device",
     "cbm_trigger_ubench", "cbm_trigger_filter_device", "cbm_trigger_build_events_device",
 )
@@ -151,6 +151,8 @@ def load_library():
         lib.cbm_trigger_fetch_selected.argtypes = [vp, u32, vp, u32, ctypes.POINTER(u32)]
         lib.cbm_trigger_select_device.restype = i32
         lib.cbm_trigger_select_device.argtypes = [vp, u32, vp, vp, vp, vp]
+        lib.cbm_trigger_select_noalloc.restype = i32
+        lib.cbm_trigger_select_noalloc.argtypes = [u32, vp, vp, vp, vp]
         lib.cbm_trigger_gather_device.restype = i32
         lib.cbm_trigger_gather_device.argtypes = [vp, u32, u64, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
         lib.cbm_trigger_msd_device.restype = i32
@@ -275,6 +277,18 @@ def cbm_trigger_fetch_selected(handle, slot, event_ids):
 def cbm_trigger_select_device(handle, n_events, d_accept, d_event_ids, d_n_selected, stream=0):
     """d_* are raw device addresses (ints); stream is a cudaStream_t as int."""
     _check(load_library().cbm_trigger_select_device(handle, n_events, d_accept, d_event_ids, d_n_selected, stream), handle)
+
+
+NOALLOC_MAX_EVENTS = 1 << 24  # CBM_TRIGGER_NOALLOC_MAX_EVENTS
+
+
+def cbm_trigger_select_noalloc(n_events, d_accept, d_event_ids, d_n_selected, stream=0):
+    """The list of selected events without a handle and without any allocation, for callers that may not allocate
+    device memory (a readout loop after start of run, a plug-in that only gets pointers and a stream): same result as
+    cbm_trigger_select_device.  d_* are raw device addresses (ints) on the current device; stream is a cudaStream_t
+    as int.  At most NOALLOC_MAX_EVENTS events; calls on one device share one fixed scratch array, so they must not
+    overlap on the GPU (include/cbm_trigger.h)."""
+    _check(load_library().cbm_trigger_select_noalloc(n_events, d_accept, d_event_ids, d_n_selected, stream), None)
 
 
 def cbm_trigger_gather_device(handle, n_events, n_hits, d_x, d_y, d_off, d_ids, d_n_sel, d_out_x, d_out_y, d_out_off,

@@ -12,6 +12,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 #include <thread>
@@ -473,8 +474,70 @@ int occupancy_grid(cbm_trigger* h, K kernel, int threads, size_t smem, int* grid
 
 }  // namespace
 
+// ---------------------------------------------------------------------------------------------- no allocation
+// cbm_trigger_select_noalloc: the selection list for callers that may not allocate (a readout loop whose device
+// memory was handed out at start of run; code that only gets pointers and a stream from its host framework).
+// The per-block counts that select_count_kernel writes and select_write_kernel reads normally sit in a cudaMalloc'ed
+// buffer of the handle (Scratch::d_selcnt).  Here they sit in this array, which is part of the library's device image:
+// the driver places one copy on every device that loads the library and keeps it until the process ends (16 KB each).
+// On the host, the name g_noalloc_block_count is only a stand-in that identifies the symbol; it is NOT the device
+// address and must never be handed to a kernel.  noalloc_block_count() asks the runtime for the real address, once
+// per device, with that device current, and hands that to the kernels.
+constexpr uint32_t kNoAllocMaxBlocks = CBM_TRIGGER_NOALLOC_MAX_EVENTS / cbm::kSelEvents;
+static_assert(CBM_TRIGGER_NOALLOC_MAX_EVENTS % cbm::kSelEvents == 0, "whole blocks");
+static __device__ __align__(256) uint32_t g_noalloc_block_count[kNoAllocMaxBlocks];
+
+namespace {
+
+constexpr int kNoAllocMaxDevices = 64;
+std::mutex g_noalloc_mutex;
+uint32_t* g_noalloc_addr[kNoAllocMaxDevices];  // device address of the array on device i; nullptr = not looked up yet
+
+// Device address of g_noalloc_block_count on the current device (looked up on the first call per device).
+int noalloc_block_count(uint32_t** out) {
+  int dev = -1;
+  CBM_CUDA(nullptr, cudaGetDevice(&dev));
+  if (dev < 0 || dev >= kNoAllocMaxDevices) return fail(nullptr, CBM_ERR_CUDA, "select_noalloc: device %d is beyond the %d this call supports", dev, kNoAllocMaxDevices);
+  std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+  if (!g_noalloc_addr[dev]) {
+    void* p = nullptr;
+    CBM_CUDA(nullptr, cudaGetSymbolAddress(&p, g_noalloc_block_count));
+    if (!p) return fail(nullptr, CBM_ERR_CUDA, "select_noalloc: cudaGetSymbolAddress returned no address");
+    g_noalloc_addr[dev] = static_cast<uint32_t*>(p);
+  }
+  *out = g_noalloc_addr[dev];
+  return CBM_OK;
+}
+
+}  // namespace
+
 // ================================================================================================ C ABI
 extern "C" {
+
+int cbm_trigger_select_noalloc(uint32_t n_events, const uint8_t* d_accept, uint32_t* d_event_ids, uint32_t* d_n_selected,
+                               void* stream) {
+  if (n_events > CBM_TRIGGER_NOALLOC_MAX_EVENTS)
+    return fail(nullptr, CBM_ERR_CAPACITY, "select_noalloc: n_events %u is above the fixed limit of %u events (the scratch of this call "
+                "is a fixed array in the library image); split the batch or use cbm_trigger_select_device", n_events,
+                CBM_TRIGGER_NOALLOC_MAX_EVENTS);
+  if (!d_n_selected || (n_events && (!d_accept || !d_event_ids)))
+    return fail(nullptr, CBM_ERR_INVALID_ARG, "select_noalloc: device pointers must not be NULL");
+  cudaStream_t st = (cudaStream_t)stream;
+  if (n_events == 0) {
+    CBM_CUDA(nullptr, cudaMemsetAsync(d_n_selected, 0, sizeof(uint32_t), st));
+    return CBM_OK;
+  }
+  uint32_t* d_block_count = nullptr;
+  const int rc = noalloc_block_count(&d_block_count);
+  if (rc) return rc;
+  // select_count_kernel writes entries 0..nb-1, select_write_kernel reads entries below its block index: every entry
+  // read was written by this call, so what an earlier call left in the array does not matter.
+  const uint32_t nb = (n_events + kSelEvents - 1) / kSelEvents;  // <= kNoAllocMaxBlocks
+  select_count_kernel<<<nb, kSelThreads, 0, st>>>(d_accept, n_events, d_block_count);
+  select_write_kernel<<<nb, kSelThreads, 0, st>>>(d_accept, n_events, d_block_count, d_event_ids, d_n_selected);
+  CBM_CUDA(nullptr, cudaGetLastError());
+  return CBM_OK;
+}
 
 #ifdef ST_DEBUG
 void cbm_trigger_debug_dump(void) {
