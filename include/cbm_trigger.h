@@ -216,8 +216,8 @@ int cbm_trigger_select_noalloc(uint32_t n_events, const uint8_t* d_accept, uint3
  * No atomics: the output is unique.  Asynchronous; uses the handle's scratch (stream-ordered calls only).
  * The list is not trusted: at most n_events entries are read, and an id >= n_events or an event whose offsets
  * off[e*L .. e*L+L] are not non-decreasing inside [0, n_hits] is gathered as an empty event.  A list that names
- * an event more than once can gather more than n_hits hits: then *d_out_n_hits (> n_hits) reports the total and
- * nothing else is written. */
+ * an event more than once can gather more than n_hits hits: then *d_out_n_hits (> n_hits) reports the total (summed
+ * in 64 bits: 2^32 hits and more are reported as they are) and nothing else is written. */
 int cbm_trigger_gather_device(cbm_trigger_t* h, uint32_t n_events, uint64_t n_hits, const int32_t* d_x, const int32_t* d_y,
                               const uint32_t* d_off, const uint32_t* d_event_ids, const uint32_t* d_n_selected,
                               int32_t* d_out_x, int32_t* d_out_y, uint32_t* d_out_off, unsigned long long* d_out_n_hits,

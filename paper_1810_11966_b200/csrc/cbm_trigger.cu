@@ -66,6 +66,7 @@ struct Scratch {
   uint32_t* d_spill[3] = {nullptr, nullptr, nullptr};  // class G, list X, class H (chain kernel); per CTA: middle-hit
                                                        // lists beyond shared memory
   uint32_t* d_selcnt = nullptr;  // accepted events per block of kSelEvents events (select.cuh)
+  unsigned long long* d_gsum = nullptr;  // hits per block of kGatherEvents list entries of the gather (select.cuh)
   uint32_t* d_hitbase = nullptr; // first hit of every selected event in the gathered batch (select.cuh)
   uint32_t* d_fcnt = nullptr;    // hits per (event, layer) of the input filter (filter.cuh), then per-block sums behind
   // station_kernel: per item (list position * S + station) the number of middle hits with triplets and the
@@ -252,6 +253,7 @@ int build_params(const cbm_trigger_config_t& c, Params& p, std::string& why) {
 int alloc_scratch(cbm_trigger* h, Scratch& s) {
   CBM_CUDA(h, cudaMalloc(&s.d_ctrl, sizeof(Ctrl)));
   CBM_CUDA(h, cudaMalloc(&s.d_selcnt, ((size_t)h->cfg.max_events / kSelEvents + 1) * sizeof(uint32_t)));
+  CBM_CUDA(h, cudaMalloc(&s.d_gsum, ((size_t)h->cfg.max_events / kGatherEvents + 1) * sizeof(unsigned long long)));
   CBM_CUDA(h, cudaMalloc(&s.d_hitbase, ((size_t)h->cfg.max_events + 1) * sizeof(uint32_t)));
   {
     const size_t n = (size_t)h->cfg.max_events * h->p.L;
@@ -273,6 +275,7 @@ int alloc_scratch(cbm_trigger* h, Scratch& s) {
 void free_scratch(Scratch& s) {
   cudaFree(s.d_ctrl);
   cudaFree(s.d_selcnt);
+  cudaFree(s.d_gsum);
   cudaFree(s.d_hitbase);
   cudaFree(s.d_fcnt);
   for (int c = 0; c < kNumLists; ++c) cudaFree(s.d_list[c]);
@@ -837,17 +840,16 @@ int cbm_trigger_gather_device(cbm_trigger_t* h, uint32_t n_events, uint64_t n_hi
   if (n_hits >= (1ull << 32)) return fail(h, CBM_ERR_CAPACITY, "n_hits must be < 2^32");
   if (!d_n_selected || !d_out_off || !d_out_n_hits || (n_events && (!d_off || !d_event_ids || !d_x || !d_y || !d_out_x || !d_out_y)))
     return fail(h, CBM_ERR_INVALID_ARG, "device pointers must not be NULL");
-  static_assert(kGatherEvents == kSelEvents, "the per-block scratch is shared with the selection list");
   CBM_CUDA(h, cudaSetDevice(h->cfg.device));
   cudaStream_t st = (cudaStream_t)stream;
   const uint32_t nb = n_events / kGatherEvents + 1;
   const Scratch& scr = h->dev_scr;
-  gather_size_kernel<<<nb, kSelThreads, 0, st>>>(d_off, h->p.L, n_events, (uint32_t)n_hits, d_event_ids, d_n_selected, scr.d_selcnt);
-  gather_base_kernel<<<nb, kSelThreads, 0, st>>>(d_off, h->p.L, n_events, (uint32_t)n_hits, d_event_ids, d_n_selected, scr.d_selcnt, scr.d_hitbase,
+  gather_size_kernel<<<nb, kSelThreads, 0, st>>>(d_off, h->p.L, n_events, (uint32_t)n_hits, d_event_ids, d_n_selected, scr.d_gsum);
+  gather_base_kernel<<<nb, kSelThreads, 0, st>>>(d_off, h->p.L, n_events, (uint32_t)n_hits, d_event_ids, d_n_selected, scr.d_gsum, scr.d_hitbase,
                                                  d_out_off, d_out_n_hits);
   if (n_events)
     gather_copy_kernel<<<h->n_sm * 8, kSelThreads, 0, st>>>(d_x, d_y, d_off, h->p.L, n_events, (uint32_t)n_hits, d_event_ids, d_n_selected,
-                                                            scr.d_hitbase, d_out_x, d_out_y, d_out_off);
+                                                            scr.d_hitbase, d_out_x, d_out_y, d_out_off, d_out_n_hits);
   CBM_CUDA(h, cudaGetLastError());
   return CBM_OK;
 }

@@ -223,3 +223,40 @@ def test_gather_device_does_not_trust_the_list():
         torch.cuda.synchronize()
         assert int(on.item()) == total
         assert int((ox != 77).sum().item()) == 0
+
+
+@pytest.mark.gpu
+def test_gather_device_repeated_ids_total_of_exactly_two_to_the_32():
+    """A list of 2^20 entries that all name one 4096-hit event gathers 2^32 hits.  The total is summed in 64 bits: a
+    32-bit sum would wrap to 0, pass the "fits the output" test and copy to wrapped positions far outside the output
+    arrays.  Required (include/cbm_trigger.h): *d_out_n_hits reports the true total and nothing else is written."""
+    import torch
+    from paper_1810_11966_b200 import binding as K
+    cfg = W.CONFIGS[0]
+    L = cfg.n_layers
+    n, big, size = 1 << 20, 12345, 4096
+    off = np.zeros(n * L + 1, dtype=np.uint32)
+    off[big * L + 1:] = size                      # event `big` holds all 4096 hits in its first layer; every other event is empty
+    rng = np.random.default_rng(5)
+    x = rng.integers(-30000, 30000, size=size + 8, dtype=np.int32)
+    with K.Trigger(cfg.layer_z, n, size, n_slots=0) as trig:
+        dx, dy = torch.from_numpy(x).cuda(), torch.from_numpy(-x).cuda()
+        do = torch.from_numpy(off.view(np.int32)).cuda()
+        dids = torch.full((n,), big, dtype=torch.int32, device="cuda")
+        dn = torch.tensor([n], dtype=torch.int32, device="cuda")
+        ox = torch.full((size + 1,), 77, dtype=torch.int32, device="cuda")
+        oy = torch.full((size + 1,), 77, dtype=torch.int32, device="cuda")
+        oo = torch.full((n * L + 1,), -1, dtype=torch.int32, device="cuda")
+        on = torch.zeros(1, dtype=torch.int64, device="cuda")
+        trig.gather_device(n, size, dx, dy, do, dids, dn, ox, oy, oo, on)
+        torch.cuda.synchronize()
+        assert int(on.item()) == n * size == 1 << 32
+        assert bool((ox == 77).all()) and bool((oy == 77).all()) and bool((oo == -1).all())
+        # the same list cut to one entry fits and is gathered (the handle is still usable)
+        dn.fill_(1)
+        trig.gather_device(n, size, dx, dy, do, dids, dn, ox, oy, oo, on)
+        torch.cuda.synchronize()
+        assert int(on.item()) == size
+        assert np.array_equal(ox.cpu().numpy()[:size], x[:size]) and int(ox[size].item()) == 77
+        o = oo.cpu().numpy().view(np.uint32)
+        assert o[:L + 1].tolist() == [0] + [size] * L
