@@ -51,6 +51,9 @@ extern "C" {
 #define CBM_TRIGGER_MAX_HITS_PER_LAYER 4096
 #define CBM_TRIGGER_MAX_SLOTS 4
 #define CBM_TRIGGER_N_KERNELS 6 /* classify, tile, class M, class H, class G, list X (see cbm_trigger_stats_t) */
+#define CBM_TRIGGER_MAX_INDEX 0xFFFFE000u /* 2^32 - 8192: largest element count of the device-side scans (records of
+                                             a stream, max_events * layers + 1); their uint32 block arithmetic (blocks of
+                                             4096 elements) cannot wrap below it */
 #define CBM_TRIGGER_PROFILE_RING 32 /* run_device calls whose per-kernel times are kept (CBM_FLAG_PROFILE) */
 
 enum {
@@ -72,7 +75,7 @@ typedef struct {
   uint32_t win_in_num, win_in_den;     /* in-station slope window a/b (half-width, closed); 0 < den <= 4096, num <= den */
   uint32_t win_link_num, win_link_den; /* cross-station window a/b, same limits */
   uint32_t min_candidates;             /* accept iff n_candidates >= this (2) */
-  uint32_t max_events;                 /* capacity of one slot, in events */
+  uint32_t max_events;                 /* capacity of one slot, in events; max_events * 3 * n_stations + 1 <= CBM_TRIGGER_MAX_INDEX */
   uint64_t max_hits;                   /* capacity of one slot, in hits; < 2^32 */
   uint32_t max_hits_per_layer;         /* 1..4096; an event with a fuller layer is rejected (CBM_ERR_RANGE) */
   uint32_t n_slots;                    /* 0..4 slots of (pinned host + device) buffers; 2 = double buffering.
@@ -232,7 +235,8 @@ int cbm_trigger_gather_device(cbm_trigger_t* h, uint32_t n_events, uint64_t n_hi
  * int32 in the worst case, 16-byte aligned and padded as for cbm_trigger_run_device) the kept hits of every event
  * grouped by layer, in stream order inside a layer (so the output is unique) -- ready for cbm_trigger_run_device on
  * the same stream.  An event with ev_off[e] > ev_off[e+1] or beyond n_records keeps nothing.  Asynchronous; no
- * atomics on global memory; uses the handle's scratch (stream-ordered calls only).  n_records < 2^32. */
+ * atomics on global memory; uses the handle's scratch (stream-ordered calls only).  n_records <= CBM_TRIGGER_MAX_INDEX, else
+ * CBM_ERR_CAPACITY. */
 int cbm_trigger_filter_device(cbm_trigger_t* h, uint32_t n_events, uint64_t n_records, const int32_t* d_xyz,
                               const uint32_t* d_ev_off, int32_t* d_out_x, int32_t* d_out_y, uint32_t* d_out_off, void* stream);
 
@@ -247,7 +251,7 @@ int cbm_trigger_filter_device(cbm_trigger_t* h, uint32_t n_events, uint64_t n_re
  * pile up into one event.  Output: d_ev_off (DEVICE, room for n_records + 1 uint32): d_ev_off[k] = first record of
  * event k, d_ev_off[*n_events] = n_records -- the d_ev_off argument of cbm_trigger_filter_device, whose output goes to
  * cbm_trigger_run_device.  *n_events (HOST) = number of events built.  Blocks until the count is on the host (the next
- * calls need it as an argument); n_records < 2^32; no atomics, the output is unique.  Scratch is allocated and freed
+ * calls need it as an argument); n_records <= CBM_TRIGGER_MAX_INDEX (else CBM_ERR_CAPACITY); no atomics, the output is unique.  Scratch is allocated and freed
  * on `stream` (cudaMallocAsync).  An event built from more than max_hits_per_layer hits in a layer is rejected by the
  * selection like any other such event (CBM_ERR_RANGE). */
 int cbm_trigger_build_events_device(cbm_trigger_t* h, uint64_t n_records, const int32_t* d_t, uint32_t t_gap,

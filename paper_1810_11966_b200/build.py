@@ -15,7 +15,7 @@ CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 LIB = os.path.join(HERE, "libcbmtrigger.so")
 SOURCES = [os.path.join(CSRC, "cbm_trigger.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, "ptx.cuh"), os.path.join(CSRC, "classify.cuh"), os.path.join(CSRC, "tile.cuh"), os.path.join(CSRC, "team.cuh"), os.path.join(CSRC, "select.cuh"), os.path.join(CSRC, "wire.cuh"), os.path.join(CSRC, "msd.cuh"), os.path.join(CSRC, "filter.cuh"), os.path.join(CSRC, "ubench.cuh"), os.path.join(CSRC, "chain.cuh"), os.path.join(CSRC, "station.cuh"), os.path.join(CSRC, "timeslice.cuh"), os.path.join(CSRC, "params.h"),
+DEPS = SOURCES + [os.path.join(CSRC, "ptx.cuh"), os.path.join(CSRC, "classify.cuh"), os.path.join(CSRC, "tile.cuh"), os.path.join(CSRC, "team.cuh"), os.path.join(CSRC, "select.cuh"), os.path.join(CSRC, "wire.cuh"), os.path.join(CSRC, "msd.cuh"), os.path.join(CSRC, "filter.cuh"), os.path.join(CSRC, "ubench.cuh"), os.path.join(CSRC, "chain.cuh"), os.path.join(CSRC, "timeslice.cuh"), os.path.join(CSRC, "params.h"),
                   os.path.join(INCLUDE, "cbm_trigger.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared", "-cudart", "static"]

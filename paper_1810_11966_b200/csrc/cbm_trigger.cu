@@ -2,7 +2,7 @@
 //
 // Owns the slots (pinned host staging, device arrays, result buffers), the three streams of the
 // H2D | kernels | D2H software pipeline ("it can be hidden by performing computation and
-// transfer in parallel") and the launch sequence of the kernels (classify, tile, team, chain, station .cuh).  No CPU fallback exists:
+// transfer in parallel") and the launch sequence of the kernels (classify, tile, team, chain .cuh).  No CPU fallback exists:
 // without a CUDA device cbm_trigger_create fails with CBM_ERR_CUDA.
 #include <cuda_runtime.h>
 
@@ -23,7 +23,6 @@
 #include "tile.cuh"
 #include "team.cuh"
 #include "chain.cuh"
-#include "station.cuh"
 #include "select.cuh"
 #include "wire.cuh"
 #include "msd.cuh"
@@ -38,20 +37,14 @@ using namespace cbm;
 // team classes (team.cuh): warps per team, fullest layer admitted, kept middle hits, coarse table (log2
 // columns, log2 rows), middle hits with triplets per station
 using SmemM = TeamSmem<1, 128, 64, 4, 4, 32>;
-using SmemH = TeamSmem<4, 448, 192, 5, 5, 48>;
 using SmemG = TeamSmem<16, 4096, 4104, 5, 5, 256>;
-constexpr int kCapM = SmemM::CAP, kCapH = SmemH::CAP, kCapG = SmemG::CAP;
-constexpr int kMinBM = 24, kMinBH = 9, kMinBG = 2;
+constexpr int kCapM = SmemM::CAP, kCapG = SmemG::CAP;
+constexpr int kMinBM = 24, kMinBG = 2;
 #define TEAM_KERNEL_M team_kernel<SmemM, kClsM, kMinBM, false, true>
-#define TEAM_KERNEL_H team_kernel<SmemH, kClsH, kMinBH, false, true>
 // class H, round-1 design (chain.cuh): 4 warps, 448 hits per layer, 32 x 32 coarse cells, 64 list entries, 8 CTAs/SM
-using SmemHC = ChainSmem<4, 448, 32, 64>;
-#define CHAIN_KERNEL_H chain_kernel<4, 448, 32, 64, kClsH, 8, true>
-// class H, one warp per (event, station) (station.cuh): 448 hits per layer, 32 x 32 coarse cells; kStWarps warps
-// per CTA, kStMinB CTAs per SM
-using SmemHS = StationSmem<448, 5, 5>;
-constexpr int kStWarps = 4, kStMinB = 5;
-#define STATION_KERNEL_H station_kernel<SmemHS, kStWarps, kClsH, kStMinB>
+constexpr int kWarpsH = 4, kCapH = 448;
+using SmemHC = ChainSmem<kWarpsH, kCapH, 32, 64>;
+#define CHAIN_KERNEL_H chain_kernel<kWarpsH, kCapH, 32, 64, kClsH, 8, true>
 #define TEAM_KERNEL_G team_kernel<SmemG, kClsG, kMinBG, true, false>
 #define TEAM_KERNEL_X team_kernel<SmemG, kClsX, kMinBG, true, false>
 // kernels of one run, in the order of cbm_trigger_stats_t::kernel_ms
@@ -69,9 +62,6 @@ struct Scratch {
   unsigned long long* d_gsum = nullptr;  // hits per block of kGatherEvents list entries of the gather (select.cuh)
   uint32_t* d_hitbase = nullptr; // first hit of every selected event in the gathered batch (select.cuh)
   uint32_t* d_fcnt = nullptr;    // hits per (event, layer) of the input filter (filter.cuh), then per-block sums behind
-  // station_kernel: per item (list position * S + station) the number of middle hits with triplets and the
-  // first kStEnt of them; per list position the number of finished stations (zero between runs)
-  uint32_t *d_st_cnt = nullptr, *d_st_ent = nullptr, *d_done = nullptr;
 };
 
 struct ProfEvents {
@@ -113,9 +103,6 @@ struct cbm_trigger {
   int n_sm = 0;
   int grid[kNumLists] = {0, 0, 0, 0};
   int grid_hc = 0;          // chain_kernel (class H)
-  int grid_hs = 0;          // station_kernel (class H)
-  int h_impl = 1;           // class H runs chain_kernel (1, default: the fastest measured), station_kernel (0) or
-                            // team_kernel (2): CBM_TRIGGER_H_IMPL=chain|station|team
   Slot slot[CBM_TRIGGER_MAX_SLOTS];
   Scratch dev_scr;          // scratch of cbm_trigger_run_device
   Ctrl* h_dev_ctrl = nullptr;
@@ -191,7 +178,9 @@ int build_params(const cbm_trigger_config_t& c, Params& p, std::string& why) {
   if (c.n_slots > CBM_TRIGGER_MAX_SLOTS) { why = "n_slots must be 0..4"; return CBM_ERR_INVALID_ARG; }
   if (c.max_events == 0) { why = "max_events must be > 0"; return CBM_ERR_INVALID_ARG; }
   if (c.max_hits >= (1ull << 32)) { why = "max_hits must be < 2^32"; return CBM_ERR_INVALID_ARG; }
-  if ((uint64_t)c.max_events * p.L + 1 >= (1ull << 32)) { why = "max_events * layers must be < 2^32"; return CBM_ERR_INVALID_ARG; }
+  // the block-wise scans index in uint32 with blocks of 4096 elements: element counts stay 8192 below 2^32 so that
+  // neither a block count nor the last block's element indices wrap (CBM_TRIGGER_MAX_INDEX)
+  if ((uint64_t)c.max_events * p.L + 1 > CBM_TRIGGER_MAX_INDEX) { why = "max_events * layers must be < 2^32 - 8192"; return CBM_ERR_INVALID_ARG; }
   if (c.tiny_max_layer_hits > kTinyMaxLayerLimit) { why = "tiny_max_layer_hits must be <= 32"; return CBM_ERR_INVALID_ARG; }
   if (c.device < 0) { why = "device must be >= 0"; return CBM_ERR_INVALID_ARG; }
 
@@ -263,13 +252,6 @@ int alloc_scratch(cbm_trigger* h, Scratch& s) {
   CBM_CUDA(h, cudaMalloc(&s.d_spill[0], (size_t)h->grid[kClsG] * 6 * kCapG * sizeof(uint32_t)));
   CBM_CUDA(h, cudaMalloc(&s.d_spill[1], (size_t)h->grid[kClsX] * 6 * kCapG * sizeof(uint32_t)));
   CBM_CUDA(h, cudaMalloc(&s.d_spill[2], (size_t)h->grid_hc * 6 * kCapH * sizeof(uint32_t)));
-  if (h->h_impl == 0) {  // scratch of station_kernel
-    const size_t n_items = (size_t)h->cfg.max_events * h->p.S;
-    CBM_CUDA(h, cudaMalloc(&s.d_st_cnt, n_items * sizeof(uint32_t)));
-    CBM_CUDA(h, cudaMalloc(&s.d_st_ent, n_items * kStEnt * sizeof(uint32_t)));
-    CBM_CUDA(h, cudaMalloc(&s.d_done, (size_t)h->cfg.max_events * sizeof(uint32_t)));
-    CBM_CUDA(h, cudaMemset(s.d_done, 0, (size_t)h->cfg.max_events * sizeof(uint32_t)));
-  }
   return CBM_OK;
 }
 void free_scratch(Scratch& s) {
@@ -280,7 +262,6 @@ void free_scratch(Scratch& s) {
   cudaFree(s.d_fcnt);
   for (int c = 0; c < kNumLists; ++c) cudaFree(s.d_list[c]);
   for (auto& sp : s.d_spill) cudaFree(sp);
-  cudaFree(s.d_st_cnt); cudaFree(s.d_st_ent); cudaFree(s.d_done);
   s = Scratch();
 }
 int make_prof(cbm_trigger* h, ProfEvents& pe) {
@@ -372,49 +353,55 @@ int launch_selection(cbm_trigger* h, const Scratch& scr, const int32_t* d_x, con
     CBM_CUDA(h, cudaEventRecord(h->ev_fork, st));
     for (auto& sd : h->st_side) CBM_CUDA(h, cudaStreamWaitEvent(sd, h->ev_fork, 0));
   }
+  // From here on the side streams hang off the caller's stream.  A CUDA error must not leave them un-joined (their
+  // kernels would run unordered against whatever the caller enqueues next, and against ev_run): the first error is
+  // kept, nothing more is launched, and the join below is still recorded and waited on before the error is returned.
+  cudaError_t err = cudaSuccess;
+  const char* err_at = "";
+#define FORKED(expr) do { if (err == cudaSuccess && (err = (expr)) != cudaSuccess) err_at = #expr; } while (0)
   // G and M first: on most workloads their persistent CTAs find a short list and leave at once
-  CBM_CUDA(h, rec(kKTeamG, 0, s_g));
-  TEAM_KERNEL_G<<<h->grid[kClsG], 32 * SmemG::W, sizeof(SmemG), s_g>>>(
-      p, d_x, d_y, d_off, d_nt, d_nc, d_ac, scr.d_ctrl, scr.d_list[kClsG], scr.d_list[kClsX], scr.d_spill[0]);
-  CBM_CUDA(h, rec(kKTeamG, 1, s_g));
-  CBM_CUDA(h, rec(kKTeamM, 0, s_m));
-  TEAM_KERNEL_M<<<h->grid[kClsM], 32 * SmemM::W, 0, s_m>>>(
-      p, d_x, d_y, d_off, d_nt, d_nc, d_ac, scr.d_ctrl, scr.d_list[kClsM], scr.d_list[kClsX], nullptr);
-  CBM_CUDA(h, rec(kKTeamM, 1, s_m));
-  CBM_CUDA(h, rec(kKTeamH, 0, st));
-  if (h->h_impl == 0) {
-    // the per-event station counters reset themselves at the end of a run; cleared here too, so that a run that was
-    // cut short cannot leave a count behind
-    CBM_CUDA(h, cudaMemsetAsync(scr.d_done, 0, (size_t)n_events * sizeof(uint32_t), st));
-    STATION_KERNEL_H<<<h->grid_hs, 32 * kStWarps, kStWarps * sizeof(SmemHS), st>>>(
-        p, d_x, d_y, d_off, d_nt, d_nc, d_ac, scr.d_ctrl, scr.d_list[kClsH], scr.d_list[kClsX], scr.d_st_cnt, scr.d_st_ent,
-        scr.d_done);
-  } else if (h->h_impl == 1)
-    CHAIN_KERNEL_H<<<h->grid_hc, 32 * SmemH::W, 0, st>>>(p, d_x, d_y, d_off, d_nt, d_nc, d_ac, scr.d_ctrl, scr.d_list[kClsH],
+  FORKED(rec(kKTeamG, 0, s_g));
+  if (err == cudaSuccess)
+    TEAM_KERNEL_G<<<h->grid[kClsG], 32 * SmemG::W, sizeof(SmemG), s_g>>>(
+        p, d_x, d_y, d_off, d_nt, d_nc, d_ac, scr.d_ctrl, scr.d_list[kClsG], scr.d_list[kClsX], scr.d_spill[0]);
+  FORKED(cudaGetLastError());
+  FORKED(rec(kKTeamG, 1, s_g));
+  FORKED(rec(kKTeamM, 0, s_m));
+  if (err == cudaSuccess)
+    TEAM_KERNEL_M<<<h->grid[kClsM], 32 * SmemM::W, 0, s_m>>>(
+        p, d_x, d_y, d_off, d_nt, d_nc, d_ac, scr.d_ctrl, scr.d_list[kClsM], scr.d_list[kClsX], nullptr);
+  FORKED(cudaGetLastError());
+  FORKED(rec(kKTeamM, 1, s_m));
+  FORKED(rec(kKTeamH, 0, st));
+  if (err == cudaSuccess)
+    CHAIN_KERNEL_H<<<h->grid_hc, 32 * kWarpsH, 0, st>>>(p, d_x, d_y, d_off, d_nt, d_nc, d_ac, scr.d_ctrl, scr.d_list[kClsH],
                                                         scr.d_spill[2]);
-  else
-    TEAM_KERNEL_H<<<h->grid[kClsH], 32 * SmemH::W, 0, st>>>(
-        p, d_x, d_y, d_off, d_nt, d_nc, d_ac, scr.d_ctrl, scr.d_list[kClsH], scr.d_list[kClsX], nullptr);
-  CBM_CUDA(h, rec(kKTeamH, 1, st));
+  FORKED(cudaGetLastError());
+  FORKED(rec(kKTeamH, 1, st));
   if (p.tiny_max_total) {
-    CBM_CUDA(h, rec(kKTile, 0, s_tile));
+    FORKED(rec(kKTile, 0, s_tile));
     const uint32_t n_tiles = (n_events + kTileEvents - 1) / kTileEvents;
-    if (p.S <= 4)  // tables sized for 4 stations: more resident CTAs
+    if (err != cudaSuccess) {
+    } else if (p.S <= 4)  // tables sized for 4 stations: more resident CTAs
       tile_kernel<4><<<n_tiles, kTileEvents * p.S, 0, s_tile>>>(p, d_x, d_y, d_off, n_events, (uint32_t)n_hits, d_nt, d_nc,
                                                                 d_ac, scr.d_ctrl, scr.d_list[kClsX]);
     else
       tile_kernel<kMaxStations><<<n_tiles, kTileEvents * p.S, 0, s_tile>>>(p, d_x, d_y, d_off, n_events, (uint32_t)n_hits, d_nt,
                                                                            d_nc, d_ac, scr.d_ctrl, scr.d_list[kClsX]);
-    CBM_CUDA(h, rec(kKTile, 1, s_tile));
+    FORKED(cudaGetLastError());
+    FORKED(rec(kKTile, 1, s_tile));
   } else if (prof) {
-    CBM_CUDA(h, rec(kKTile, 0, s_tile));
-    CBM_CUDA(h, rec(kKTile, 1, s_tile));
+    FORKED(rec(kKTile, 0, s_tile));
+    FORKED(rec(kKTile, 1, s_tile));
   }
   if (!serial)
-    for (int i = 0; i < 3; ++i) {
-      CBM_CUDA(h, cudaEventRecord(h->ev_join[i], h->st_side[i]));
-      CBM_CUDA(h, cudaStreamWaitEvent(st, h->ev_join[i], 0));
+    for (int i = 0; i < 3; ++i) {  // always, also after an error above
+      cudaError_t e1 = cudaEventRecord(h->ev_join[i], h->st_side[i]);
+      if (e1 == cudaSuccess) e1 = cudaStreamWaitEvent(st, h->ev_join[i], 0);
+      if (err == cudaSuccess && e1 != cudaSuccess) { err = e1; err_at = "join of the side streams"; }
     }
+#undef FORKED
+  if (err != cudaSuccess) return fail(h, CBM_ERR_CUDA, "%s: %s", err_at, cudaGetErrorString(err));
   CBM_CUDA(h, rec(kKTeamX, 0, st));
   TEAM_KERNEL_X<<<h->grid[kClsX], 32 * SmemG::W, sizeof(SmemG), st>>>(
       p, d_x, d_y, d_off, d_nt, d_nc, d_ac, scr.d_ctrl, scr.d_list[kClsX], scr.d_list[kClsX], scr.d_spill[1]);
@@ -542,17 +529,6 @@ int cbm_trigger_select_noalloc(uint32_t n_events, const uint8_t* d_accept, uint3
   return CBM_OK;
 }
 
-#ifdef ST_DEBUG
-void cbm_trigger_debug_dump(void) {
-  unsigned long long v[16];
-  cudaDeviceSynchronize();
-  cudaMemcpyFromSymbol(v, cbm::g_st_dbg, sizeof(v));
-  printf("ST_DEBUG rounds %llu surv %llu d2passes %llu d2items %llu joiners %llu mc0 %llu mc2 %llu slow %llu cand %llu allcand %llu over3 %llu\n", v[0], v[1], v[2], v[3], v[4], v[5], v[6], v[7], v[8], v[9], v[10]);
-  memset(v, 0, sizeof(v));
-  cudaMemcpyToSymbol(cbm::g_st_dbg, v, sizeof(v));
-}
-#endif
-
 const char* cbm_trigger_version(void) { return "cbm-trigger 0.2 sm_100a"; }
 
 const char* cbm_trigger_last_error(const cbm_trigger_t* h) { return h ? h->err.c_str() : g_create_err.c_str(); }
@@ -589,17 +565,11 @@ int cbm_trigger_create(const cbm_trigger_config_t* cfg, cbm_trigger_t** out) {
   CREATE_CUDA(cudaGetDeviceProperties(&prop, cfg->device));
   if (prop.major < 10) { fail(h, CBM_ERR_CUDA, "device is sm_%d%d; this library holds sm_100a code only", prop.major, prop.minor); return bail(CBM_ERR_CUDA); }
   h->n_sm = prop.multiProcessorCount;
-  static_assert(sizeof(SmemM) <= 48 * 1024 && sizeof(SmemH) <= 48 * 1024 && sizeof(SmemHC) <= 48 * 1024, "static shared memory limit");
+  static_assert(sizeof(SmemM) <= 48 * 1024 && sizeof(SmemHC) <= 48 * 1024, "static shared memory limit");
   CREATE_CUDA(cudaFuncSetAttribute(tile_kernel<4>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
   CREATE_CUDA(cudaFuncSetAttribute(tile_kernel<kMaxStations>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
   CREATE_TRY(occupancy_grid(h, TEAM_KERNEL_M, 32 * SmemM::W, 0, &h->grid[kClsM]));
-  CREATE_TRY(occupancy_grid(h, TEAM_KERNEL_H, 32 * SmemH::W, 0, &h->grid[kClsH]));
-  CREATE_TRY(occupancy_grid(h, CHAIN_KERNEL_H, 32 * SmemH::W, 0, &h->grid_hc));
-  CREATE_TRY(occupancy_grid(h, STATION_KERNEL_H, 32 * kStWarps, kStWarps * sizeof(SmemHS), &h->grid_hs));
-  {
-    const char* impl = getenv("CBM_TRIGGER_H_IMPL");  // tuning: the other two kernels for class H
-    h->h_impl = (impl && strcmp(impl, "team") == 0) ? 2 : (impl && strcmp(impl, "station") == 0) ? 0 : 1;
-  }
+  CREATE_TRY(occupancy_grid(h, CHAIN_KERNEL_H, 32 * kWarpsH, 0, &h->grid_hc));
   CREATE_TRY(occupancy_grid(h, TEAM_KERNEL_G, 32 * SmemG::W, sizeof(SmemG), &h->grid[kClsG]));
   CREATE_TRY(occupancy_grid(h, TEAM_KERNEL_X, 32 * SmemG::W, sizeof(SmemG), &h->grid[kClsX]));
   CREATE_CUDA(cudaStreamCreateWithFlags(&h->st_h2d, cudaStreamNonBlocking));
@@ -858,7 +828,7 @@ int cbm_trigger_filter_device(cbm_trigger_t* h, uint32_t n_events, uint64_t n_re
                               const uint32_t* d_ev_off, int32_t* d_out_x, int32_t* d_out_y, uint32_t* d_out_off, void* stream) {
   if (!h) return CBM_ERR_INVALID_ARG;
   if (n_events > h->cfg.max_events) return fail(h, CBM_ERR_CAPACITY, "n_events %u > max_events %u", n_events, h->cfg.max_events);
-  if (n_records >= (1ull << 32)) return fail(h, CBM_ERR_CAPACITY, "n_records must be < 2^32");
+  if (n_records > CBM_TRIGGER_MAX_INDEX) return fail(h, CBM_ERR_CAPACITY, "n_records must be <= 2^32 - 8192");
   if (!d_out_off || (n_events && (!d_ev_off || (n_records && (!d_xyz || !d_out_x || !d_out_y)))))
     return fail(h, CBM_ERR_INVALID_ARG, "device pointers must not be NULL");
   CBM_CUDA(h, cudaSetDevice(h->cfg.device));
@@ -887,7 +857,7 @@ int cbm_trigger_build_events_device(cbm_trigger_t* h, uint64_t n_records, const 
                                     uint32_t* n_events, void* stream) {
   if (!h) return CBM_ERR_INVALID_ARG;
   if (!n_events || !d_ev_off || (n_records && !d_t)) return fail(h, CBM_ERR_INVALID_ARG, "pointers must not be NULL");
-  if (n_records >= (1ull << 32)) return fail(h, CBM_ERR_CAPACITY, "n_records must be < 2^32");
+  if (n_records > CBM_TRIGGER_MAX_INDEX) return fail(h, CBM_ERR_CAPACITY, "n_records must be <= 2^32 - 8192");
   cudaStream_t st = (cudaStream_t)stream;
   CBM_CUDA(h, cudaSetDevice(h->cfg.device));
   *n_events = 0;
@@ -896,7 +866,8 @@ int cbm_trigger_build_events_device(cbm_trigger_t* h, uint64_t n_records, const 
     CBM_CUDA(h, cudaStreamSynchronize(st));
     return CBM_OK;
   }
-  const uint32_t n = (uint32_t)n_records;
+  static_assert(kSelEvents <= 4096 && kFlagThreads <= 4096, "CBM_TRIGGER_MAX_INDEX leaves room for one block of 4096 and one of 4096");
+  const uint32_t n = (uint32_t)n_records;                   // <= 2^32 - 8192: the sums below do not wrap
   const uint32_t nb = (n + kSelEvents - 1) / kSelEvents;
   // scratch of this call (stream-ordered allocation): the flags, the per-block counts of the compaction, the count
   uint8_t* d_flag = nullptr;
@@ -987,10 +958,17 @@ int cbm_trigger_ubench(cbm_trigger_t* h, cbm_trigger_ubench_t* out) {
   CBM_CUDA(h, cudaSetDevice(h->cfg.device));
   const int grid = h->n_sm * kUbCtasPerSm;
   uint32_t* d_out = nullptr;
-  CBM_CUDA(h, cudaMalloc(&d_out, (size_t)grid * kUbThreads * sizeof(uint32_t)));
-  cudaEvent_t e0, e1;
-  CBM_CUDA(h, cudaEventCreate(&e0));
-  CBM_CUDA(h, cudaEventCreate(&e1));
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  // every exit, also a failing one, releases the buffer and the two events
+  auto done = [&](cudaError_t e, const char* what) {
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+    cudaFree(d_out);
+    return e == cudaSuccess ? CBM_OK : fail(h, CBM_ERR_CUDA, "ubench: %s: %s", what, cudaGetErrorString(e));
+  };
+  cudaError_t err = cudaMalloc(&d_out, (size_t)grid * kUbThreads * sizeof(uint32_t));
+  if (err != cudaSuccess) return done(err, "cudaMalloc");
+  if ((err = cudaEventCreate(&e0)) != cudaSuccess || (err = cudaEventCreate(&e1)) != cudaSuccess) return done(err, "cudaEventCreate");
   const double lanes = (double)grid * kUbThreads * (double)kUbIter * 8.0;  // chain steps of one launch
   auto timed = [&](int which, double* per_s, double per_step) -> cudaError_t {
     float best = 1e30f;
@@ -1012,15 +990,12 @@ int cbm_trigger_ubench(cbm_trigger_t* h, cbm_trigger_ubench_t* out) {
     *per_s = lanes * per_step / (best * 1e-3);
     return cudaGetLastError();
   };
-  CBM_CUDA(h, timed(0, &out->alu_lane_ops_per_s, 2.0));      // IADD3 + LOP3
-  CBM_CUDA(h, timed(1, &out->imad_lane_ops_per_s, 1.0));     // IMAD
-  CBM_CUDA(h, timed(2, &out->window_evals_per_s, 1.0));      // one evaluation = x and y
-  CBM_CUDA(h, timed(3, &out->packed_tests_per_s, 1.0));
+  if ((err = timed(0, &out->alu_lane_ops_per_s, 2.0)) != cudaSuccess) return done(err, "alu kernel");        // IADD3 + LOP3
+  if ((err = timed(1, &out->imad_lane_ops_per_s, 1.0)) != cudaSuccess) return done(err, "imad kernel");      // IMAD
+  if ((err = timed(2, &out->window_evals_per_s, 1.0)) != cudaSuccess) return done(err, "window kernel");     // one evaluation = x and y
+  if ((err = timed(3, &out->packed_tests_per_s, 1.0)) != cudaSuccess) return done(err, "packed kernel");
   out->n_sm = (uint32_t)h->n_sm;
-  cudaEventDestroy(e0);
-  cudaEventDestroy(e1);
-  cudaFree(d_out);
-  return CBM_OK;
+  return done(cudaSuccess, "");
 }
 
 int cbm_trigger_device_status(cbm_trigger_t* h, void* stream, cbm_trigger_stats_t* stats) {

@@ -81,6 +81,9 @@ def _cfg(**kw):
     (lambda c: setattr(c, "n_slots", 5), "n_slots"),
     (lambda c: setattr(c, "max_events", 0), "max_events"),
     (lambda c: setattr(c, "max_hits", 1 << 32), "max_hits"),
+    # 12 layers: max_events * 12 + 1 one step above CBM_TRIGGER_MAX_INDEX = 2^32 - 8192 (the uint32 block arithmetic of
+    # the device scans must not wrap)
+    (lambda c: setattr(c, "max_events", 0xFFFFE000 // 12 + 1), "max_events * layers"),
     (lambda c: setattr(c, "tiny_max_layer_hits", 33), "tiny_max_layer_hits"),
 ])
 def test_create_rejects_bad_config_before_cuda(lib, mutate, needle):

@@ -124,3 +124,24 @@ def test_build_events_device_small_cases():
             ne = trig.build_events_device(n, dt, gap, deo)
             assert ne == want.size - 1
             assert np.array_equal(deo.cpu().numpy().view(np.uint32)[:ne + 1], want)
+
+
+@pytest.mark.gpu
+def test_record_count_limit_is_checked_before_anything_runs():
+    """include/cbm_trigger.h: n_records <= CBM_TRIGGER_MAX_INDEX = 2^32 - 8192 for the stream calls (above it the
+    uint32 block arithmetic of the scans would wrap and truncate the output silently); refused with CBM_ERR_CAPACITY."""
+    import torch
+    from paper_1810_11966_b200 import binding as K
+    small = torch.zeros(16, dtype=torch.int32, device="cuda")
+    with K.Trigger([60000, 70000, 80000], 16, 16, n_slots=0) as trig:
+        for n_records in (0xFFFFE000 + 1, 2**32 - 1, 2**32):
+            with pytest.raises(K.CbmTriggerError) as ei:
+                trig.build_events_device(n_records, small, 4, small)
+            assert ei.value.code == K.CBM_ERR_CAPACITY
+            with pytest.raises(K.CbmTriggerError) as ei:
+                trig.filter_device(1, n_records, small, small, small, small, small)
+            assert ei.value.code == K.CBM_ERR_CAPACITY
+        # the handle is still usable
+        t = torch.tensor([1, 2, 9], dtype=torch.int32, device="cuda")
+        eo = torch.full((4,), -1, dtype=torch.int32, device="cuda")
+        assert trig.build_events_device(3, t, 4, eo) == 2 and eo.cpu().tolist()[:3] == [0, 2, 3]
