@@ -33,26 +33,6 @@ def oracle_mt(geo, x, y, off, e_begin=0, e_end=None, n_threads=None, chunk=2000)
     return nt, nc, ac
 
 
-def oracle_list_mt(geo, x, y, off, ids, n_threads=None):
-    ids = np.asarray(ids, dtype=np.uint64)
-    S = geo.n_stations
-    n_threads = n_threads or min(32, os.cpu_count() or 1)
-    parts = np.array_split(np.arange(ids.size), max(1, min(ids.size, n_threads * 4)))
-    nt = np.zeros((ids.size, S), dtype=np.uint32)
-    nc = np.zeros(ids.size, dtype=np.uint32)
-    ac = np.zeros(ids.size, dtype=np.uint8)
-
-    def work(p):
-        if p.size == 0:
-            return
-        t, c, k = oracle.run_list(geo, x, y, off, ids[p])
-        nt[p], nc[p], ac[p] = t, c, k
-
-    with ThreadPoolExecutor(n_threads) as ex:
-        list(ex.map(work, parts))
-    return nt, nc, ac
-
-
 def gpu_select(layer_z, x, y, off, win_in=(1, 100), win_link=(2, 100), min_candidates=2, max_hits_per_layer=4096,
                flags=0, tiny_max_layer_hits=0, check=True):
     """One batch through cbm_trigger_create / upload_events / run / fetch_results."""
@@ -125,13 +105,3 @@ def device_run(cfg, b, flags=0):
         rc, st = trig.device_status()
         assert rc == K.CBM_OK
     return (dnt.cpu().numpy().view(np.uint32).reshape(-1, S), dnc.cpu().numpy().view(np.uint32), dac.cpu().numpy(), st.as_dict())
-
-
-def parity_sample(b, cfg, nc, ac, fraction, seed=99, h_cap=448):
-    """Event ids to recompute with the oracle when all of them would take too long: a seeded fraction of the batch,
-    every event with a candidate, every accepted event and every event of the heaviest class (a layer above h_cap)."""
-    E, L = b.n_events, cfg.n_layers
-    rng = np.random.default_rng(seed)
-    mx = np.diff(b.off.astype(np.int64)).reshape(E, L).max(axis=1)
-    return np.unique(np.concatenate([rng.choice(E, size=int(E * fraction), replace=False), np.flatnonzero(nc > 0),
-                                     np.flatnonzero(ac), np.flatnonzero(mx > h_cap)]))
