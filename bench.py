@@ -40,7 +40,14 @@ if ROOT not in sys.path:
 METRIC = "events_per_second"
 UNIT = "events/s"
 CBM_INTERACTION_RATE_HZ = 1.0e7
-TRAFFIC_CSV = os.path.join("profiles", "r2_traffic.csv")  # ncu --set full captures, per kernel and workload
+TRAFFIC_CSV = os.path.join("profiles", "r3_traffic.csv")  # ncu --set full captures, per kernel and workload
+INST_CSV = os.path.join("profiles", "r3_inst.csv")
+# the source files a kernel is compiled from (beside the shared ptx.cuh / params.h / classify.cuh): a committed ncu
+# figure is quoted as this run's only while these files are byte-identical to the ones the capture was taken from
+KERNEL_SOURCES = {"classify_kernel": ("classify.cuh",), "tile_kernel": ("tile.cuh",), "team_kernel_M": ("team.cuh",),
+                  "chain_kernel_H": ("chain.cuh",), "team_kernel_G": ("team.cuh",), "team_kernel_X": ("team.cuh",),
+                  "msd_kernel": ("msd.cuh",)}
+SHARED_SOURCES = ("ptx.cuh", "params.h", "classify.cuh")
 
 
 def parse_args():
@@ -76,31 +83,51 @@ def measured_peaks():
     return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
 
 
+def kernel_source_sha(kernel):
+    """First 16 hex digits of the SHA-256 over the files `kernel` is compiled from (KERNEL_SOURCES + SHARED_SOURCES,
+    in that order).  The ncu CSVs under profiles/ store the value of the build they were captured from; .git does not
+    travel to the GPU box, so this - not a commit id - is what the bench can check at run time."""
+    import hashlib
+    h = hashlib.sha256()
+    csrc = os.path.join(ROOT, "paper_1810_11966_b200", "csrc")
+    for fn in KERNEL_SOURCES.get(kernel, ()) + SHARED_SOURCES:
+        with open(os.path.join(csrc, fn), "rb") as f:
+            h.update(f.read())
+    return h.hexdigest()[:16]
+
+
+def _capture_row(row, kernel):
+    """Provenance of one committed ncu figure; "stale" = the kernel's sources changed since the capture."""
+    sha = row.get("source_sha16") or ""
+    return {"kind": "committed_capture", "capture": row.get("capture"), "commit": row.get("commit"), "source_sha16": sha,
+            "stale": sha != kernel_source_sha(kernel)}
+
+
 def ncu_traffic(workload, kernel):
     """dram__bytes_read.sum + dram__bytes_write.sum of one committed `ncu --set full` capture of this kernel on
-    this workload (profiles/r2_traffic.csv names the capture and the commit it was taken at), else None."""
+    this workload (profiles/r3_traffic.csv names the capture, its commit and the hash of the kernel's sources), else
+    None.  A figure whose kernel sources have changed since is returned with "stale": True and must not be quoted."""
     path = os.path.join(ROOT, TRAFFIC_CSV)
     if not os.path.exists(path):
         return None
     with open(path) as f:
         for row in csv.DictReader(f):
             if row.get("workload") == workload and row.get("kernel") == kernel:
-                return {"bytes": int(row["dram_bytes_read"]) + int(row["dram_bytes_write"]), "source": TRAFFIC_CSV,
-                        "capture": row.get("capture"), "commit": row.get("commit")}
+                return dict(_capture_row(row, kernel), bytes=int(row["dram_bytes_read"]) + int(row["dram_bytes_write"]),
+                            source=TRAFFIC_CSV)
     return None
 
 
 def ncu_instructions(workload):
     """smsp__inst_executed.sum of the committed `ncu --set full` captures of this workload's kernels
-    (profiles/r2_inst.csv names capture and commit): {kernel: warp-instructions per launch}."""
-    path = os.path.join(ROOT, "profiles/r2_inst.csv")
+    (profiles/r3_inst.csv): {kernel: warp-instructions per launch, provenance, "stale"}."""
+    path = os.path.join(ROOT, INST_CSV)
     res = {}
     if os.path.exists(path):
         with open(path) as f:
             for row in csv.DictReader(f):
                 if row.get("workload") == workload:
-                    res[row["kernel"]] = {"warp_instructions": int(row["warp_instructions"]), "capture": row.get("capture"),
-                                          "commit": row.get("commit")}
+                    res[row["kernel"]] = dict(_capture_row(row, row["kernel"]), warp_instructions=int(row["warp_instructions"]))
     return res
 
 
@@ -449,7 +476,8 @@ def run_ours(args, cfg, cid):
     achieved = kbytes[dom] / (dom_ms * 1e-3) / 1e9 if dom_ms > 0 else 0.0
     traffic = ncu_traffic(cfg.name, K.KERNEL_NAMES[dom])
     roofline = {"bound": "hbm", "kernel": K.KERNEL_NAMES[dom], "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": traffic["bytes"] if traffic else None, "traffic_source": traffic,
+                "frac": achieved / peak, "traffic": traffic["bytes"] if traffic and not traffic["stale"] else None,
+                "traffic_source": traffic,  # a committed capture, not a counter of this run; null above when stale
                 "peak_source": peak_src, "algorithmic_bytes_per_launch": kbytes[dom], "ms_per_launch": dom_ms,
                 "share_of_serial_step": dom_ms / float(kmean.sum()) if kmean.sum() > 0 else None,
                 "timing": "CUDA events around the kernel on its stream, kernels launched one after the other (CBM_FLAG_SERIAL)"}
@@ -465,9 +493,13 @@ def run_ours(args, cfg, cid):
                    "launch": "serial" if args.serial else "side by side"},
         "hits_per_second": hits_all * args.steps / (ms_total_max * 1e-3),
         "vs_10MHz": value / CBM_INTERACTION_RATE_HZ,
-        "gpu_launches": K.N_KERNELS * args.steps,
+        # kernels launched in the timed region: the library's own count of the last run (cbm_trigger_stats_t.n_launches),
+        # the same for every step of a fixed batch
+        "gpu_launches": int(stats["n_launches"]) * args.steps,
         "kernels": {name: {"ms": float(kmean[i]), "events": acct[i]["events"], "hits": acct[i]["hits"],
-                           "algorithmic_bytes": kbytes[i]} for i, name in enumerate(K.KERNEL_NAMES)},
+                           "algorithmic_bytes": kbytes[i],
+                           "frac": kbytes[i] / (float(kmean[i]) * 1e-3) / 1e9 / peak if kmean[i] > 0 else None}
+                    for i, name in enumerate(K.KERNEL_NAMES)},
         "serial_step_ms": float(kmean.sum()),
         "classes": stats["n_class"], "events_redone": stats["n_redone"], "accepted_events": n_accept,
         "events_with_candidates": n_cand_events,
@@ -478,7 +510,7 @@ def run_ours(args, cfg, cid):
     }
     # What the kernels are bound by in fact: instruction issue.  The warp-instructions of the
     # captured kernels of this workload (committed ncu captures) at one instruction per scheduler and cycle.
-    inst = ncu_instructions(cfg.name)
+    inst = {k: v for k, v in ncu_instructions(cfg.name).items() if not v["stale"]}
     if inst and clocks.get("sm_mhz"):
         n_sched = 4 * torch.cuda.get_device_properties(local_rank).multi_processor_count
         wi = sum(v["warp_instructions"] for v in inst.values())
@@ -486,7 +518,9 @@ def run_ours(args, cfg, cid):
         out["roofline_step"]["issue"] = {
             "warp_instructions_per_step": wi, "kernels": inst, "schedulers": n_sched, "sm_mhz": clocks["sm_mhz"],
             "t_issue_ms": t_issue_ms, "frac": t_issue_ms / ms_per_step,
-            "note": "captured kernels only; the step cannot be shorter than t_issue_ms at this instruction count"}
+            "kind": "committed_capture",
+            "note": "instruction counts from committed ncu captures whose kernel sources are unchanged (not counters of "
+                    "this run); captured kernels only; the step cannot be shorter than t_issue_ms at this instruction count"}
     if ubench:
         out["ubench"] = dict(ubench, note="cbm_trigger_ubench: measured on this GPU in this run, 8 chains per thread")
     if e2e:
@@ -654,6 +688,7 @@ def run_msd(args):
     peak, peak_src = measured_peaks()
     B_alg = 8 * n_hits + 4 * (E * L + 1) + 5 * E  # hits, offsets, n_passing + accept
     gbs = B_alg / (ms_per_step * 1e-3) / 1e9
+    msd_traffic = ncu_traffic(cfg.name, "msd_kernel")
     out = {
         "metric": METRIC, "value": value, "value_kind": "hbm_resident", "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -664,7 +699,8 @@ def run_msd(args):
         "hits_per_second": hits_all * args.steps / (ms_total_max * 1e-3), "vs_10MHz": value / CBM_INTERACTION_RATE_HZ,
         "gpu_launches": args.steps, "accepted_events": int(dac.sum().item()),
         "roofline": {"bound": "hbm", "kernel": "msd_kernel", "achieved": gbs, "peak": peak, "unit": "GB/s", "frac": gbs / peak,
-                     "traffic": None, "peak_source": peak_src, "algorithmic_bytes_per_launch": B_alg, "ms_per_launch": ms_per_step},
+                     "traffic": msd_traffic["bytes"] if msd_traffic and not msd_traffic["stale"] else None,
+                     "traffic_source": msd_traffic, "peak_source": peak_src, "algorithmic_bytes_per_launch": B_alg, "ms_per_launch": ms_per_step},
         "paper_context": {"gpu_events_per_s": 2.84e5, "gpu": "Tesla C2075, 40 000 events (PAPER.md:220, Table 1)",
                           "cpu_events_per_s_1_thread": 6.25e4, "cpu": "Xeon 2.8 GHz, one core (PAPER.md:213-221)",
                           "note": "other hardware, the paper's own data sample: context, not a baseline"},
@@ -683,8 +719,27 @@ def run_msd(args):
     print(json.dumps(out))
 
 
+def self_launch_command(argv, n_gpus, port):
+    """`python bench.py --gpus N ...` started without a launcher: the command that starts the N ranks (one per GPU of this
+    node, rendezvous on 127.0.0.1), each of which runs this script again with the same arguments.  Events are
+    independent, so the ranks are replicas with their own event ranges; NCCL carries the barrier and the max-reduction of
+    the times only."""
+    return [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={n_gpus}",
+            "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + list(argv)
+
+
+def free_port():
+    import socket
+    with socket.socket() as sock:
+        sock.bind(("127.0.0.1", 0))
+        return sock.getsockname()[1]
+
+
 def main():
     args = parse_args()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ and args.impl == "ours":
+        import subprocess
+        raise SystemExit(subprocess.call(self_launch_command(sys.argv[1:], args.gpus, free_port())))
     from paper_1810_11966_b200 import workloads as W
     cfg = W.CONFIGS[args.config]
     if args.impl == "reference":
