@@ -147,6 +147,13 @@ int cbm_trigger_host_buffers_packed(cbm_trigger_t* h, uint32_t slot, uint8_t** x
 int cbm_trigger_upload_events_packed(cbm_trigger_t* h, uint32_t slot, uint32_t n_events, uint64_t n_hits,
                                      const uint8_t* xy20, const uint32_t* off);
 
+/* The producer side of XY20, for a C caller (host code, no CUDA, no handle): writes hit i of x[] / y[] (HOST, int32)
+ * to out[5*i .. 5*i+4] (HOST, n_hits*5 bytes; may be a slot's buffer from cbm_trigger_host_buffers_packed).
+ * Returns CBM_OK, CBM_ERR_INVALID_ARG for a NULL pointer with n_hits > 0, or CBM_ERR_RANGE if a coordinate lies
+ * outside [-524288, 524287]: then *first_bad (HOST, may be NULL) is the smallest such hit index and the bytes of the
+ * hits before it have been written.  On success *first_bad is n_hits. */
+int cbm_trigger_pack_xy20(const int32_t* x, const int32_t* y, uint64_t n_hits, uint8_t* out, uint64_t* first_bad);
+
 /* a3-a8: enqueue the selection kernels for the batch in `slot` after its H2D, and the D2H of the results after
  * the kernels (separate streams, event-ordered).  Returns immediately.
  * PAPER.md:162-163 "launch the kernel ... events are processed in parallel". */

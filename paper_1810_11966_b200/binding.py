@@ -25,7 +25,7 @@ EXPORTS = (
     "cbm_trigger_get_stats", "cbm_trigger_last_error", "cbm_trigger_version", "cbm_trigger_device_kernel_times",
     "cbm_trigger_fetch_selected", "cbm_trigger_select_device", "cbm_trigger_select_noalloc",
     "cbm_trigger_host_buffers_packed", "cbm_trigger_upload_events_packed", "cbm_trigger_msd_device", "cbm_trigger_gather_device",
-    "cbm_trigger_ubench", "cbm_trigger_filter_device", "cbm_trigger_build_events_device",
+    "cbm_trigger_ubench", "cbm_trigger_filter_device", "cbm_trigger_build_events_device", "cbm_trigger_pack_xy20",
 )
 PROFILE_RING = 32
 # scheduler classes (csrc/cbm_trigger.cu, csrc/params.h), restated for bookkeeping in bench.py only
@@ -151,6 +151,8 @@ def load_library():
         lib.cbm_trigger_fetch_selected.argtypes = [vp, u32, vp, u32, ctypes.POINTER(u32)]
         lib.cbm_trigger_select_device.restype = i32
         lib.cbm_trigger_select_device.argtypes = [vp, u32, vp, vp, vp, vp]
+        lib.cbm_trigger_pack_xy20.restype = i32
+        lib.cbm_trigger_pack_xy20.argtypes = [vp, vp, u64, vp, ctypes.POINTER(u64)]
         lib.cbm_trigger_select_noalloc.restype = i32
         lib.cbm_trigger_select_noalloc.argtypes = [u32, vp, vp, vp, vp]
         lib.cbm_trigger_gather_device.restype = i32
@@ -277,6 +279,23 @@ def cbm_trigger_fetch_selected(handle, slot, event_ids):
 def cbm_trigger_select_device(handle, n_events, d_accept, d_event_ids, d_n_selected, stream=0):
     """d_* are raw device addresses (ints); stream is a cudaStream_t as int."""
     _check(load_library().cbm_trigger_select_device(handle, n_events, d_accept, d_event_ids, d_n_selected, stream), handle)
+
+
+def cbm_trigger_pack_xy20(x, y, out=None):
+    """The library's host packer of the wire format XY20 (no CUDA): int32 numpy arrays -> 5 bytes per hit.  `out` may be
+    a slot's pinned buffer (cbm_trigger_host_buffers_packed).  Raises CbmTriggerError(CBM_ERR_RANGE) for a coordinate
+    outside the 20-bit range; the exception carries `first_bad`."""
+    n = int(x.size)
+    if out is None:
+        out = np.empty(5 * n, dtype=np.uint8)
+    assert out.dtype == np.uint8 and out.flags.c_contiguous and out.size >= 5 * n
+    bad = ctypes.c_uint64(0)
+    rc = load_library().cbm_trigger_pack_xy20(_host_ptr(x, np.int32), _host_ptr(y, np.int32), n, out.ctypes.data, ctypes.byref(bad))
+    if rc != CBM_OK:
+        err = CbmTriggerError(rc, cbm_trigger_last_error(None))
+        err.first_bad = int(bad.value)
+        raise err
+    return out[:5 * n]
 
 
 NOALLOC_MAX_EVENTS = 1 << 24  # CBM_TRIGGER_NOALLOC_MAX_EVENTS

@@ -704,6 +704,24 @@ int cbm_trigger_upload_events_packed(cbm_trigger_t* h, uint32_t slot, uint32_t n
   return CBM_OK;
 }
 
+int cbm_trigger_pack_xy20(const int32_t* x, const int32_t* y, uint64_t n_hits, uint8_t* out, uint64_t* first_bad) {
+  if (first_bad) *first_bad = n_hits;
+  if (n_hits && (!x || !y || !out)) return fail(nullptr, CBM_ERR_INVALID_ARG, "pack_xy20: x, y, out must not be NULL");
+  constexpr int32_t kMin = -(1 << 19), kMax = (1 << 19) - 1;
+  for (uint64_t i = 0; i < n_hits; ++i) {
+    const int32_t xv = x[i], yv = y[i];
+    if (xv < kMin || xv > kMax || yv < kMin || yv > kMax) {
+      if (first_bad) *first_bad = i;
+      return fail(nullptr, CBM_ERR_RANGE, "pack_xy20: hit %llu (%d, %d) is outside the 20-bit range of XY20", (unsigned long long)i, xv, yv);
+    }
+    // bits 0..19 = x, bits 20..39 = y (two's complement), little endian
+    const uint64_t v = ((uint64_t)(uint32_t)xv & 0xFFFFFu) | (((uint64_t)(uint32_t)yv & 0xFFFFFu) << 20);
+    uint8_t* o = out + 5 * i;
+    o[0] = (uint8_t)v; o[1] = (uint8_t)(v >> 8); o[2] = (uint8_t)(v >> 16); o[3] = (uint8_t)(v >> 24); o[4] = (uint8_t)(v >> 32);
+  }
+  return CBM_OK;
+}
+
 int cbm_trigger_run(cbm_trigger_t* h, uint32_t slot) {
   int rc = check_slot(h, slot);
   if (rc) return rc;

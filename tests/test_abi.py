@@ -27,7 +27,7 @@ def declared_symbols():
         if fn.endswith(".h"):
             text = open(os.path.join(inc, fn)).read()
             text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
-            names |= set(re.findall(r"\b(cbm_trigger_[a-z_]+)\s*\(", text))
+            names |= set(re.findall(r"\b(cbm_trigger_[a-z0-9_]+)\s*\(", text))
     return sorted(names)
 
 

@@ -41,6 +41,32 @@ def test_pack_unpack_round_trip_and_limits():
             W.pack_xy20(np.array([0], np.int32), np.array([bad], np.int32))
 
 
+def test_library_packer_against_the_oracle_decoder_and_hand_written_bytes():
+    """cbm_trigger_pack_xy20 (host code of the C library, no CUDA): hand-written byte strings, a round trip through
+    oracle.unpack_xy20 (the format's definition), the range limits with the index of the first bad hit."""
+    from paper_1810_11966_b200 import binding as K
+    # the hand cases of test_unpack_hand_written_bytes, in the packing direction
+    p = K.cbm_trigger_pack_xy20(np.array([1, 0, -1], np.int32), np.array([0, 1, -1], np.int32))
+    assert bytes(p) == bytes([1, 0, 0, 0, 0, 0, 0, 0x10, 0, 0, 0xFF, 0xFF, 0xFF, 0xFF, 0xFF])
+    assert bytes(K.cbm_trigger_pack_xy20(np.array([524287], np.int32), np.array([-524288], np.int32))) == bytes([0xFF, 0xFF, 0x07, 0x00, 0x80])
+    assert bytes(K.cbm_trigger_pack_xy20(np.array([0x12345], np.int32), np.array([0x0ABCD], np.int32))) == bytes([0x45, 0x23, 0xD1, 0xBC, 0x0A])
+    assert K.cbm_trigger_pack_xy20(np.zeros(0, np.int32), np.zeros(0, np.int32)).size == 0
+    rng = np.random.default_rng(8)
+    for n in (1, 3, 4, 5, 1001):
+        x = rng.integers(W.XY20_MIN, W.XY20_MAX + 1, size=n, dtype=np.int32)
+        y = rng.integers(W.XY20_MIN, W.XY20_MAX + 1, size=n, dtype=np.int32)
+        out = np.full(5 * n + 3, 0xAB, dtype=np.uint8)
+        p = K.cbm_trigger_pack_xy20(x, y, out)
+        ux, uy = oracle.unpack_xy20(p)
+        assert np.array_equal(ux, x) and np.array_equal(uy, y)
+        assert (out[5 * n:] == 0xAB).all()  # nothing written past the end
+    for bad in (W.XY20_MAX + 1, W.XY20_MIN - 1, 2**31 - 1, -2**31):
+        for xs, ys in (([5, 6, bad, 7], [1, 2, 3, 4]), ([5, 6, 7, 8], [1, 2, bad, bad])):
+            with pytest.raises(K.CbmTriggerError) as ei:
+                K.cbm_trigger_pack_xy20(np.array(xs, np.int32), np.array(ys, np.int32))
+            assert ei.value.code == K.CBM_ERR_RANGE and ei.value.first_bad == 2
+
+
 def test_workload_coordinates_fit_the_format():
     for cid in (0, 1, 2, 3):
         b = W.generate(W.CONFIGS[cid], n_events=300)
